@@ -1,0 +1,247 @@
+/*
+ * smre_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded fp64 CPU statement of what the hot path of
+ * arXiv 1503.03492 computes: Dykstra's projection of a residual image onto the
+ * intersection of the window balls  ||x_S||^2 <= c_S  (Eq. 5),
+ * in the standard form (Alg. 2) and in the paper's
+ * "incomplete" form (Sec. 3.2 + Listing 2/3).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference leg may call this file.  It shares no code, header, table
+ * or helper with the CUDA path under paper_1503_03492_b200/csrc/.
+ *
+ * Notation: thresholds c_S = 1 / c_s(alpha) of the paper;
+ * increment sign  v = x + q  (q here = -q of Alg. 2; negation is exact).
+ *
+ * Every loop below is window-serial and in the order the paper / DESIGN.md
+ * readings state; no blocking, fusion or reordering.
+ *
+ * Pins (tests/test_oracle_*.py): closed-form single ball (Eq. 14), identity on
+ * feasible input, one-family == one projection, side-1 == clip, conservation
+ * x + sum_f q_f == y, feasibility in the limit, variational inequality, KKT
+ * structure, SLSQP brute force on tiny images, box-cap-ball closed form,
+ * symmetries, ICD == composition of restricted standard runs == explicit
+ * tile-by-tile solve, counts.  No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ---------------------------------------------------------------------------
+ * One window step.  Eq. 14 with c_S = 1/c_s:
+ *     p_s(v) = v * sqrt(c_S / ||v||^2)  if ||v||^2 > c_S   (strict, A5)
+ *              v                         else
+ * applied to v = x + q (Listing 3: s1 = e - q, paper sign), then
+ * q' = v - p_s(v)   (Listing 3, PAPER.md:502 + 510: q = -s1; q += s1_scaled).
+ * The sum of squares runs row-major over the window.
+ * Returns 1 when the window was scaled (constraint active), else 0.
+ * ------------------------------------------------------------------------- */
+static int window_step(double *x, double *q, int W, int wy, int wx, int s, double c)
+{
+    double n2 = 0.0;
+    for (int r = wy; r < wy + s; ++r)
+        for (int col = wx; col < wx + s; ++col) {
+            double v = x[(size_t)r * W + col] + q[(size_t)r * W + col];
+            n2 += v * v;
+        }
+    double alpha = 1.0;
+    int active = 0;
+    if (n2 > c) {
+        alpha = sqrt(c / n2);
+        active = 1;
+    }
+    for (int r = wy; r < wy + s; ++r)
+        for (int col = wx; col < wx + s; ++col) {
+            size_t i = (size_t)r * W + col;
+            double v = x[i] + q[i];
+            double xn = alpha * v;
+            q[i] = v - xn;
+            x[i] = xn;
+        }
+    return active;
+}
+
+/* One family pass: every window of side s with origin == (oy, ox) mod s that
+ * lies fully inside the H x W image (reading A6).  The windows of a family are
+ * disjoint, so their order is irrelevant; row-major here. */
+static long long family_pass(double *x, double *q, int H, int W,
+                             int s, int oy, int ox, double c)
+{
+    long long n_active = 0;
+    for (int wy = oy; wy + s <= H; wy += s)
+        for (int wx = ox; wx + s <= W; wx += s)
+            n_active += window_step(x, q, W, wy, wx, s, c);
+    return n_active;
+}
+
+/* ---------------------------------------------------------------------------
+ * Cyclic Dykstra over an explicit ordered family list (Alg. 2, PAPER.md:178,
+ * read as A1/A2: one step per set, sets visited cyclically, one sweep = one
+ * pass over the list).  q_f = 0 initially for every f.
+ *   y      : H*W row-major input
+ *   fam_*  : F entries: side, row offset, column offset, threshold
+ *   x_out  : H*W result
+ *   q_out  : NULL, or F*H*W increments after the last sweep (plane f = family f)
+ *   n_active_last : NULL, or number of scaled windows during the last sweep
+ * Returns 0, or -1 on allocation failure / bad arguments.
+ * ------------------------------------------------------------------------- */
+int smre_oracle_dykstra_families(const double *y, int H, int W,
+                                 const int *fam_side, const int *fam_oy,
+                                 const int *fam_ox, const double *fam_c, int F,
+                                 int n_sweeps, double *x_out, double *q_out,
+                                 long long *n_active_last)
+{
+    if (!y || !x_out || H <= 0 || W <= 0 || F < 0 || n_sweeps < 0) return -1;
+    size_t N = (size_t)H * W;
+    double *q = q_out;
+    if (!q) {
+        q = (double *)malloc(sizeof(double) * N * (size_t)(F > 0 ? F : 1));
+        if (!q) return -1;
+    }
+    memset(q, 0, sizeof(double) * N * (size_t)F);
+    if (x_out != y) memcpy(x_out, y, sizeof(double) * N);
+    long long act = 0;
+    for (int sweep = 0; sweep < n_sweeps; ++sweep) {
+        act = 0;
+        for (int f = 0; f < F; ++f)
+            act += family_pass(x_out, q + (size_t)f * N, H, W,
+                               fam_side[f], fam_oy[f], fam_ox[f], fam_c[f]);
+    }
+    if (n_active_last) *n_active_last = act;
+    if (!q_out) free(q);
+    return 0;
+}
+
+/* Number of families of the standard ("exact") method: sum of s^2. */
+int smre_oracle_std_family_count(const int *sides, int n_sides)
+{
+    int F = 0;
+    for (int a = 0; a < n_sides; ++a) F += sides[a] * sides[a];
+    return F;
+}
+
+/* Canonical family order, reading A3: sides[] as given, then oy ascending,
+ * then ox ascending.  Arrays must hold smre_oracle_std_family_count entries. */
+void smre_oracle_std_family_list(const int *sides, const double *c, int n_sides,
+                                 int *fam_side, int *fam_oy, int *fam_ox, double *fam_c)
+{
+    int f = 0;
+    for (int a = 0; a < n_sides; ++a)
+        for (int oy = 0; oy < sides[a]; ++oy)
+            for (int ox = 0; ox < sides[a]; ++ox) {
+                fam_side[f] = sides[a];
+                fam_oy[f] = oy;
+                fam_ox[f] = ox;
+                fam_c[f] = c[a];
+                ++f;
+            }
+}
+
+/* ---------------------------------------------------------------------------
+ * Algorithm O-STD: the "exact method" window set, all square
+ * windows of every side in sides[] at every shift, n_sweeps
+ * sweeps in the canonical order.  q_out: NULL or F*H*W.
+ * ------------------------------------------------------------------------- */
+int smre_oracle_std(const double *y, int H, int W, const int *sides, const double *c,
+                    int n_sides, int n_sweeps, double *x_out, double *q_out,
+                    long long *n_active_last)
+{
+    if (!sides || !c || n_sides <= 0) return -1;
+    int F = smre_oracle_std_family_count(sides, n_sides);
+    int *fs = (int *)malloc(sizeof(int) * 3 * (size_t)F);
+    double *fc = (double *)malloc(sizeof(double) * (size_t)F);
+    if (!fs || !fc) { free(fs); free(fc); return -1; }
+    smre_oracle_std_family_list(sides, c, n_sides, fs, fs + F, fs + 2 * F, fc);
+    int rc = smre_oracle_dykstra_families(y, H, W, fs, fs + F, fs + 2 * F, fc, F,
+                                          n_sweeps, x_out, q_out, n_active_last);
+    free(fs);
+    free(fc);
+    return rc;
+}
+
+/* ---------------------------------------------------------------------------
+ * Algorithm O-ICD, the paper's incomplete Dykstra:
+ *   window collection: squares of edge 2^k, k <= K, shifted by
+ *   2^i "in each direction" (diagonal, Listing 2 PAPER.md:393,
+ *   reading A-ICD-4/5);  Omega^i = all levels k >= i at shift 2^i
+ *   (union of collections, reading A-ICD-1);
+ *   P_incomplete = product over i = 0..K of P_{Omega^i} (PAPER.md:377,
+ *   A-ICD-2), applied i ascending (Listing 2, A-ICD-3).
+ * Each P_{Omega^i} is a Dykstra run from q = 0 (Listing 3 PAPER.md:431-433,
+ * A-ICD-9) over the levels K, K-1, ..., i in that order (PAPER.md:453,
+ * A-ICD-10), repeated n_sweeps times (reading A-ICD-8: the paper's
+ * "while delta > tol*1024" loop is replaced by a fixed count).
+ * Borders (A-ICD-13): a level is the tiling of the whole plane with origin
+ * (2^i mod 2^k) on the diagonal, restricted to windows fully inside the image.
+ *
+ *   level_c[k] : threshold of side 2^k, k = 0..K
+ * ------------------------------------------------------------------------- */
+int smre_oracle_icd_levels(const double *y, int H, int W, int K, const double *level_c,
+                           int n_sweeps, double *x_out)
+{
+    if (!y || !x_out || !level_c || H <= 0 || W <= 0 || K < 0 || K > 30 || n_sweeps < 0)
+        return -1;
+    size_t N = (size_t)H * W;
+    double *q = (double *)malloc(sizeof(double) * N * (size_t)(K + 1));
+    if (!q) return -1;
+    if (x_out != y) memcpy(x_out, y, sizeof(double) * N);
+    for (int i = 0; i <= K; ++i) {                    /* shift loop, Listing 2 */
+        int shift = 1 << i;
+        memset(q, 0, sizeof(double) * N * (size_t)(K + 1));   /* "Set q = 0" */
+        for (int cyc = 0; cyc < n_sweeps; ++cyc)
+            for (int k = K; k >= i; --k) {            /* for (s = 5; s >= smin; s--) */
+                int side = 1 << k;
+                int o = shift % side;                  /* offset (o, o) */
+                family_pass(x_out, q + (size_t)k * N, H, W, side, o, o, level_c[k]);
+            }
+    }
+    free(q);
+    return 0;
+}
+
+/* Front end taking the same (sides, c) table as the standard variant:
+ * K = floor(log2(max side)) (Eq. 21, reading A-ICD-6); every 2^k,
+ * k <= K, must be present in sides[] (else -2); other sides are ignored
+ * (reading A-ICD-7). */
+int smre_oracle_icd(const double *y, int H, int W, const int *sides, const double *c,
+                    int n_sides, int n_sweeps, double *x_out)
+{
+    if (!sides || !c || n_sides <= 0) return -1;
+    int smax = 0;
+    for (int a = 0; a < n_sides; ++a) if (sides[a] > smax) smax = sides[a];
+    if (smax < 1) return -1;
+    int K = 0;
+    while ((2 << K) <= smax) ++K;
+    double level_c[32];
+    for (int k = 0; k <= K; ++k) {
+        int found = 0;
+        for (int a = 0; a < n_sides; ++a)
+            if (sides[a] == (1 << k)) { level_c[k] = c[a]; found = 1; break; }
+        if (!found) return -2;
+    }
+    return smre_oracle_icd_levels(y, H, W, K, level_c, n_sweeps, x_out);
+}
+
+/* ---------------------------------------------------------------------------
+ * Sum of squares of EVERY s x s window fully inside the image (all shifts),
+ * by direct summation: out[(H-s+1)*(W-s+1)], out[wy*(W-s+1)+wx] = t_s of the
+ * window with origin (wy, wx)  (t_s).  Used by the tests to form
+ * the violated-window sets of the parity protocol.
+ * ------------------------------------------------------------------------- */
+int smre_oracle_window_sums(const double *x, int H, int W, int s, double *out)
+{
+    if (!x || !out || s < 1 || s > H || s > W) return -1;
+    int nwy = H - s + 1, nwx = W - s + 1;
+    for (int wy = 0; wy < nwy; ++wy)
+        for (int wx = 0; wx < nwx; ++wx) {
+            double n2 = 0.0;
+            for (int r = wy; r < wy + s; ++r)
+                for (int col = wx; col < wx + s; ++col) {
+                    double v = x[(size_t)r * W + col];
+                    n2 += v * v;
+                }
+            out[(size_t)wy * nwx + wx] = n2;
+        }
+    return 0;
+}

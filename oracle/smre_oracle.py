@@ -1,0 +1,179 @@
+"""ctypes front end of oracle/smre_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+leg may import this module.  It never imports paper_1503_03492_b200 and shares
+nothing with the CUDA path.
+
+Every function takes float32 or float64 numpy arrays, up-casts them to float64
+(readings A10: the fp32 threshold *values* are up-cast, so both sides compare
+against numerically identical thresholds) and returns float64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "smre_oracle.c")
+_LIB = os.path.join(_HERE, "libsmre_oracle.so")
+
+# Flags are part of the timed CPU baseline: -O2, no fast-math.
+CFLAGS = ["-O2", "-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra"]
+
+
+def build(force: bool = False) -> str:
+    """Compile smre_oracle.c with gcc into oracle/libsmre_oracle.so."""
+    stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+    if force or stale:
+        subprocess.check_call(["gcc", *CFLAGS, "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+_dp = ctypes.POINTER(ctypes.c_double)
+_ip = ctypes.POINTER(ctypes.c_int)
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.smre_oracle_dykstra_families.restype = ctypes.c_int
+        lib.smre_oracle_dykstra_families.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, _ip, _ip, _ip, _dp, ctypes.c_int,
+            ctypes.c_int, _dp, _dp, ctypes.POINTER(ctypes.c_longlong)]
+        lib.smre_oracle_std.restype = ctypes.c_int
+        lib.smre_oracle_std.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, _ip, _dp, ctypes.c_int, ctypes.c_int,
+            _dp, _dp, ctypes.POINTER(ctypes.c_longlong)]
+        lib.smre_oracle_std_family_count.restype = ctypes.c_int
+        lib.smre_oracle_std_family_count.argtypes = [_ip, ctypes.c_int]
+        lib.smre_oracle_std_family_list.restype = None
+        lib.smre_oracle_std_family_list.argtypes = [_ip, _dp, ctypes.c_int, _ip, _ip, _ip, _dp]
+        lib.smre_oracle_icd_levels.restype = ctypes.c_int
+        lib.smre_oracle_icd_levels.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_int, _dp]
+        lib.smre_oracle_icd.restype = ctypes.c_int
+        lib.smre_oracle_icd.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, _ip, _dp, ctypes.c_int, ctypes.c_int, _dp]
+        lib.smre_oracle_window_sums.restype = ctypes.c_int
+        lib.smre_oracle_window_sums.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
+        _lib = lib
+    return _lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a), dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(np.asarray(a), dtype=np.int32)
+
+
+def _p(a, t):
+    return a.ctypes.data_as(t)
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"{what} failed with code {rc}")
+
+
+def std_family_list(sides, c):
+    """Canonical ordered family list [(side, oy, ox, c)] of the exact method (A3)."""
+    lib = _load()
+    sides = _i32(sides)
+    c = _f64(c)
+    F = lib.smre_oracle_std_family_count(_p(sides, _ip), len(sides))
+    fs, fy, fx = (np.zeros(F, np.int32) for _ in range(3))
+    fc = np.zeros(F, np.float64)
+    lib.smre_oracle_std_family_list(_p(sides, _ip), _p(c, _dp), len(sides),
+                                    _p(fs, _ip), _p(fy, _ip), _p(fx, _ip), _p(fc, _dp))
+    return [(int(a), int(b), int(d), float(e)) for a, b, d, e in zip(fs, fy, fx, fc)]
+
+
+def dykstra_families(y, families, n_sweeps, return_q=False, return_active=False):
+    """Cyclic Dykstra (Alg. 2) over an explicit ordered list [(side, oy, ox, c)]."""
+    lib = _load()
+    y = _f64(y)
+    assert y.ndim == 2
+    H, W = y.shape
+    F = len(families)
+    fs = _i32([f[0] for f in families])
+    fy = _i32([f[1] for f in families])
+    fx = _i32([f[2] for f in families])
+    fc = _f64([f[3] for f in families])
+    x = np.empty_like(y)
+    q = np.zeros((F, H, W), np.float64) if return_q else None
+    act = ctypes.c_longlong(0)
+    rc = lib.smre_oracle_dykstra_families(
+        _p(y, _dp), H, W, _p(fs, _ip), _p(fy, _ip), _p(fx, _ip), _p(fc, _dp), F,
+        int(n_sweeps), _p(x, _dp), _p(q, _dp) if return_q else None, ctypes.byref(act))
+    _check(rc, "smre_oracle_dykstra_families")
+    out = (x,)
+    if return_q:
+        out += (q,)
+    if return_active:
+        out += (act.value,)
+    return out if len(out) > 1 else x
+
+
+def project_std(y, sides, c, n_sweeps, return_q=False):
+    """Algorithm O-STD on one image [H,W] or a stack [B,H,W] (frames independent)."""
+    lib = _load()
+    y = _f64(y)
+    sides = _i32(sides)
+    c = _f64(c)
+    if y.ndim == 3:
+        res = [project_std(f, sides, c, n_sweeps, return_q) for f in y]
+        if return_q:
+            return np.stack([r[0] for r in res]), np.stack([r[1] for r in res], axis=1)
+        return np.stack(res)
+    H, W = y.shape
+    x = np.empty_like(y)
+    q = None
+    if return_q:
+        F = lib.smre_oracle_std_family_count(_p(sides, _ip), len(sides))
+        q = np.zeros((F, H, W), np.float64)
+    rc = lib.smre_oracle_std(_p(y, _dp), H, W, _p(sides, _ip), _p(c, _dp), len(sides),
+                             int(n_sweeps), _p(x, _dp), _p(q, _dp) if return_q else None, None)
+    _check(rc, "smre_oracle_std")
+    return (x, q) if return_q else x
+
+
+def project_icd(y, sides, c, n_sweeps):
+    """Algorithm O-ICD on one image [H,W] or a stack [B,H,W] (frames independent)."""
+    lib = _load()
+    y = _f64(y)
+    sides = _i32(sides)
+    c = _f64(c)
+    if y.ndim == 3:
+        return np.stack([project_icd(f, sides, c, n_sweeps) for f in y])
+    H, W = y.shape
+    x = np.empty_like(y)
+    rc = lib.smre_oracle_icd(_p(y, _dp), H, W, _p(sides, _ip), _p(c, _dp), len(sides),
+                             int(n_sweeps), _p(x, _dp))
+    _check(rc, "smre_oracle_icd")
+    return x
+
+
+def project(y, sides, c, n_sweeps, variant):
+    if variant in ("standard", 0):
+        return project_std(y, sides, c, n_sweeps)
+    if variant in ("incomplete", 1):
+        return project_icd(y, sides, c, n_sweeps)
+    raise ValueError(variant)
+
+
+def window_sums(x, s):
+    """t_s of every s x s window fully inside the image, all shifts: [(H-s+1),(W-s+1)]."""
+    lib = _load()
+    x = _f64(x)
+    H, W = x.shape
+    out = np.empty((H - s + 1, W - s + 1), np.float64)
+    _check(lib.smre_oracle_window_sums(_p(x, _dp), H, W, int(s), _p(out, _dp)),
+           "smre_oracle_window_sums")
+    return out
