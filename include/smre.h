@@ -1,0 +1,132 @@
+/*
+ * smre.h -- C ABI of the B200-native Dykstra projection onto multi-scale window balls
+ * (the hot path of arXiv 1503.03492, "Parallel Statistical Multi-resolution Estimation").
+ *
+ * What it computes.  Given a residual image y (the argument X of P_G in Eq. 12-13,
+ * PAPER.md:159-164) the library runs Dykstra's algorithm (Alg. 2) with the
+ * closed-form ball projection of Eq. 14 onto the sets
+ *        tau_S = { x : sum_{i in S} x_i^2 <= c_S }          (Eq. 5)
+ * for square windows S.  c_S here is a THRESHOLD: c_S = 1 / c_s(alpha) of the paper.
+ *
+ *   SMRE_STANDARD   -- the paper's "exact method" (Sec. 3.1; window set of
+ *                      Fig. 5): every square window of every side in sides[], at
+ *                      every shift, fully inside the image.  Windows sharing (side, oy, ox) are
+ *                      disjoint (one "family") and are projected in parallel;
+ *                      families run in the fixed order sides[] as given, then oy ascending, then
+ *                      ox ascending.  One sweep = one pass over all sum(side^2) families.  One
+ *                      fp32 increment plane q_f per family lives in device memory.
+ *   SMRE_INCOMPLETE -- the paper's "incomplete Dykstra" (Sec. 3.2, Listing
+ *                      2/3): K = floor(log2(max side)); for shift i = 0..K ascending, a Dykstra
+ *                      run from q = 0 over the nested tilings of side 2^K, ..., 2^i (coarse to
+ *                      fine) whose origin is (2^i mod side) on the diagonal; n_sweeps inner cycles
+ *                      per shift.  Increments never leave the chip.
+ *
+ * All arithmetic is fp32, IEEE round-to-nearest, no fast-math; the
+ * comparison is strict (project iff sum > c_S, Eq. 14).  Images are dense row-major
+ * [batch][H][W] fp32, idx = (b*H + row)*W + col, frames independent.
+ *
+ * Threading / streams.  Every call returns a status; nothing is thrown across the ABI.
+ * smre_project only ENQUEUES work on the caller's CUDA stream: no host synchronisation, no host
+ * round-trip between families.  One in-flight smre_project per handle.  Each call starts from
+ * q = 0 (Alg. 2: q_{0,s} = 0); no state carries between calls.
+ *
+ * There is no CPU path: without a CUDA device smre_create fails with SMRE_ECUDA.
+ */
+#ifndef SMRE_H
+#define SMRE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct smre_handle_s *smre_handle;
+
+typedef enum {
+    SMRE_OK = 0,
+    SMRE_EINVAL = 1,        /* null pointer, non-positive size, side < 1 or > min(H,W), duplicate side,
+                               non-positive threshold, missing power-of-two level for SMRE_INCOMPLETE */
+    SMRE_EUNSUPPORTED = 2,  /* side beyond the compiled limit (SMRE_MAX_SIDE), unknown schedule */
+    SMRE_ENOMEM = 3,        /* device allocation of the increment planes / workspace failed */
+    SMRE_ECUDA = 4          /* any other CUDA runtime error (text in smre_last_error) */
+} smre_status;
+
+typedef enum { SMRE_STANDARD = 0, SMRE_INCOMPLETE = 1 } smre_variant;
+
+/* How the ordered family sequence of SMRE_STANDARD is driven (the "sweep scheduler"). */
+typedef enum {
+    SMRE_SCHED_AUTO = 0,        /* persistent if the image tiles fit on chip, else graph */
+    SMRE_SCHED_GRAPH = 1,       /* one kernel per family, one captured CUDA graph per sweep */
+    SMRE_SCHED_PERSISTENT = 2   /* one cooperative kernel per call: x tiles resident in shared
+                                   memory, q streamed from HBM, neighbour hand-off between CTAs */
+} smre_schedule;
+
+#define SMRE_MAX_SIDE 32        /* largest window side (the paper's L_SMRE = 32) */
+
+/*
+ * Create a solver for [batch][H][W] images.
+ *   out      (host, out)  receives the handle; owned by the caller until smre_destroy.
+ *   sides    (host, in)   n_sides distinct window sides, 1 <= side <= min(H, W, SMRE_MAX_SIDE);
+ *                         their order is the family order of SMRE_STANDARD.
+ *   c_table  (host, in)   n_sides thresholds c_S > 0, c_table[a] belongs to sides[a].
+ *   variant               SMRE_INCOMPLETE needs every 2^k, k <= floor(log2(max side)), in sides[];
+ *                         other sides are ignored by it.
+ * Allocates (device): SMRE_STANDARD  sum(side^2)*batch*H*W*4 bytes of increment planes plus a
+ * batch*H*W*4 work image and a small mailbox workspace; SMRE_INCOMPLETE nothing of image size.
+ * The arrays sides / c_table are copied; the caller may free them on return.
+ */
+smre_status smre_create(smre_handle *out, int H, int W, int batch,
+                        const int *sides, int n_sides, const float *c_table,
+                        smre_variant variant);
+
+/*
+ * Project.  y_dev, x_out_dev: DEVICE pointers to batch*H*W contiguous fp32.  y_dev is only read;
+ * x_out_dev == y_dev (in place) is allowed (the paper's kernels work in place on e,
+ * PAPER.md:516).  n_sweeps >= 1: sweeps (standard) / inner cycles per shift (incomplete).
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous.
+ */
+smre_status smre_project(smre_handle h, const float *y_dev, float *x_out_dev,
+                         int n_sweeps, void *cuda_stream);
+
+/*
+ * Same projection with HOST buffers (pageable or pinned): copies y to the device, projects,
+ * copies the result back, all on cuda_stream, and returns after the stream has drained.
+ * The staging buffers belong to the handle.
+ */
+smre_status smre_project_host(smre_handle h, const float *y_host, float *x_out_host,
+                              int n_sweeps, void *cuda_stream);
+
+/* Frees every device and host resource of the handle.  NULL is accepted. */
+smre_status smre_destroy(smre_handle h);
+
+/* ---- diagnostics and test hooks (not on the hot path) -------------------------------------- */
+
+/* Select the sweep scheduler of SMRE_STANDARD (default SMRE_SCHED_AUTO).  SMRE_EUNSUPPORTED if
+ * the persistent schedule cannot hold this image on chip. */
+smre_status smre_set_schedule(smre_handle h, smre_schedule schedule);
+
+/* n_families: families per sweep (standard) / level passes per inner cycle summed over shifts
+ * (incomplete).  windows_per_sweep: windows visited per sweep / per inner cycle, all frames.
+ * increment_bytes: device bytes held for q.  Any pointer may be NULL. */
+smre_status smre_info(smre_handle h, int *n_families, long long *windows_per_sweep,
+                      long long *increment_bytes);
+
+/* Family idx in execution order: side, row offset oy, column offset ox, threshold.  For
+ * SMRE_INCOMPLETE idx runs over the level passes (shift-major), oy == ox. */
+smre_status smre_family(smre_handle h, int idx, int *side, int *oy, int *ox, float *c);
+
+/* SMRE_STANDARD only: copy the increment planes of the last smre_project to q_out_dev,
+ * layout [F][batch][H][W] fp32 (device pointer).  Asynchronous on cuda_stream. */
+smre_status smre_export_increments(smre_handle h, float *q_out_dev, void *cuda_stream);
+
+/* Scheduler actually used by the last smre_project (smre_schedule value), number of kernels it
+ * launched, and the persistent schedule's tile grid (0 x 0 if unused).  Pointers may be NULL. */
+smre_status smre_last_launch(smre_handle h, int *schedule_used, long long *kernel_launches,
+                             int *tiles_y, int *tiles_x);
+
+/* Text of the last error on the calling thread ("" if none).  Never NULL. */
+const char *smre_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SMRE_H */

@@ -1,0 +1,45 @@
+// Shared declarations of the CUDA path (sm_100a).  Not used by, and shares nothing with, oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace smre {
+
+struct Family {
+    int side, oy, ox;   // windows of edge `side` with origin == (oy, ox) mod side
+    int ny, nx;         // floor((H-oy)/side), floor((W-ox)/side): windows fully inside (reading A6)
+    float c;            // threshold c_S = 1/c_s(alpha)                                 (Eq. 5)
+    float sqrt_c;       // sqrtf(c), rounded once on the host
+};
+
+// Eq. 14 in threshold form: scale factor alpha = sqrt(c/n2) of a window whose sum
+// of squares is n2, 1 when the window is inside its ball.  Strict compare (reading A5).
+// Default: sqrt(c) * rsqrt(n2) with the hardware reciprocal square root (MUFU.RSQ, <= 2 ulp):
+// branch-free and ~4x shorter on the dependent chain that bounds a family step than IEEE
+// division + square root.  -DSMRE_PRECISE_SCALE selects sqrt_rn(div_rn(c, n2)) for A/B checks.
+// Every scheduler and both variants use this one function, so they agree bit for bit.
+__device__ __forceinline__ float ball_scale(float n2, float c, float sqrt_c) {
+#ifdef SMRE_PRECISE_SCALE
+    (void)sqrt_c;
+    return (n2 > c) ? __fsqrt_rn(__fdiv_rn(c, n2)) : 1.0f;
+#else
+    return (n2 > c) ? sqrt_c * rsqrtf(n2) : 1.0f;
+#endif
+}
+
+// ---- launchers implemented in the .cu files --------------------------------------------------
+
+// smre_family.cu: one family pass over all frames (schedule SMRE_SCHED_GRAPH).
+cudaError_t launch_family_pass(float *x, float *q_plane, int B, int H, int W, const Family &f,
+                               cudaStream_t st);
+
+// smre_icd.cu: one shift of the incomplete Dykstra (P_{Omega^i}).
+struct IcdLevels {
+    float c[6];         // c[k]: threshold of side 2^k, k = 0..K
+    float sqrt_c[6];
+};
+// src may equal dst.  K <= 5.
+cudaError_t launch_icd_shift(const float *src, float *dst, int B, int H, int W, int K, int shift_i,
+                             const IcdLevels &lv, int n_cycles, cudaStream_t st);
+
+}  // namespace smre

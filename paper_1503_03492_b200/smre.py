@@ -1,0 +1,190 @@
+"""ctypes binding of include/smre.h: same names, argument marshalling only.
+
+Every step of the projection runs in the CUDA kernels behind the C ABI.  There is no CPU
+fallback: if libsmre.so is missing or cannot be loaded, importing callers get an exception.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import _build
+
+SMRE_OK, SMRE_EINVAL, SMRE_EUNSUPPORTED, SMRE_ENOMEM, SMRE_ECUDA = range(5)
+SMRE_STANDARD, SMRE_INCOMPLETE = 0, 1
+SMRE_SCHED_AUTO, SMRE_SCHED_GRAPH, SMRE_SCHED_PERSISTENT = 0, 1, 2
+_STATUS = {0: "SMRE_OK", 1: "SMRE_EINVAL", 2: "SMRE_EUNSUPPORTED", 3: "SMRE_ENOMEM", 4: "SMRE_ECUDA"}
+
+# every symbol include/smre.h declares
+exported_symbols = (
+    "smre_create", "smre_project", "smre_project_host", "smre_destroy", "smre_set_schedule",
+    "smre_info", "smre_family", "smre_export_increments", "smre_last_launch", "smre_last_error",
+)
+
+
+class SmreError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"{_STATUS.get(status, status)}: {text}")
+        self.status = status
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+_lib = None
+_vp, _ip, _fp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_float)
+_llp = ctypes.POINTER(ctypes.c_longlong)
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen libsmre.so (building it with nvcc first if the sources are newer)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build() if build_if_missing else _build.LIB
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: build it with `python -m paper_1503_03492_b200._build`")
+    lib = ctypes.CDLL(path)
+    lib.smre_create.argtypes = [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                _ip, ctypes.c_int, _fp, ctypes.c_int]
+    lib.smre_project.argtypes = [_vp, _vp, _vp, ctypes.c_int, _vp]
+    lib.smre_project_host.argtypes = [_vp, _vp, _vp, ctypes.c_int, _vp]
+    lib.smre_destroy.argtypes = [_vp]
+    lib.smre_set_schedule.argtypes = [_vp, ctypes.c_int]
+    lib.smre_info.argtypes = [_vp, _ip, _llp, _llp]
+    lib.smre_family.argtypes = [_vp, ctypes.c_int, _ip, _ip, _ip, _fp]
+    lib.smre_export_increments.argtypes = [_vp, _vp, _vp]
+    lib.smre_last_launch.argtypes = [_vp, _ip, _llp, _ip, _ip]
+    for name in exported_symbols:
+        getattr(lib, name).restype = ctypes.c_int
+    lib.smre_last_error.restype = ctypes.c_char_p
+    lib.smre_last_error.argtypes = []
+    _lib = lib
+    return lib
+
+
+def smre_last_error() -> str:
+    return load_library().smre_last_error().decode()
+
+
+def _check(status):
+    if status != SMRE_OK:
+        raise SmreError(status, smre_last_error())
+
+
+def smre_create(H, W, batch, sides, c_table, variant):
+    """-> opaque handle (int).  sides: ints, c_table: float32 thresholds, one per side."""
+    lib = load_library()
+    sides = np.ascontiguousarray(sides, dtype=np.int32)
+    c_table = np.ascontiguousarray(c_table, dtype=np.float32)
+    if sides.ndim != 1 or sides.shape != c_table.shape:
+        raise ValueError("sides and c_table must be 1-D and of equal length")
+    h = _vp()
+    _check(lib.smre_create(ctypes.byref(h), int(H), int(W), int(batch),
+                           sides.ctypes.data_as(_ip), len(sides), c_table.ctypes.data_as(_fp),
+                           int(variant)))
+    return h.value
+
+
+def smre_project(handle, y_ptr, x_out_ptr, n_sweeps, stream=0):
+    """y_ptr / x_out_ptr: device addresses (tensor.data_ptr()); stream: cudaStream_t as int."""
+    _check(load_library().smre_project(handle, y_ptr, x_out_ptr, int(n_sweeps), stream))
+
+
+def smre_project_host(handle, y_ptr, x_out_ptr, n_sweeps, stream=0):
+    """Host addresses (numpy .ctypes.data or pinned tensor.data_ptr()); blocks until done."""
+    _check(load_library().smre_project_host(handle, y_ptr, x_out_ptr, int(n_sweeps), stream))
+
+
+def smre_destroy(handle):
+    _check(load_library().smre_destroy(handle))
+
+
+def smre_set_schedule(handle, schedule):
+    _check(load_library().smre_set_schedule(handle, int(schedule)))
+
+
+def smre_info(handle):
+    n, w, b = ctypes.c_int(), ctypes.c_longlong(), ctypes.c_longlong()
+    _check(load_library().smre_info(handle, ctypes.byref(n), ctypes.byref(w), ctypes.byref(b)))
+    return n.value, w.value, b.value
+
+
+def smre_family(handle, idx):
+    s, oy, ox, c = ctypes.c_int(), ctypes.c_int(), ctypes.c_int(), ctypes.c_float()
+    _check(load_library().smre_family(handle, int(idx), ctypes.byref(s), ctypes.byref(oy),
+                                      ctypes.byref(ox), ctypes.byref(c)))
+    return s.value, oy.value, ox.value, c.value
+
+
+def smre_export_increments(handle, q_out_ptr, stream=0):
+    _check(load_library().smre_export_increments(handle, q_out_ptr, stream))
+
+
+def smre_last_launch(handle):
+    s, n, ty, tx = ctypes.c_int(), ctypes.c_longlong(), ctypes.c_int(), ctypes.c_int()
+    _check(load_library().smre_last_launch(handle, ctypes.byref(s), ctypes.byref(n),
+                                           ctypes.byref(ty), ctypes.byref(tx)))
+    return s.value, n.value, ty.value, tx.value
+
+
+class Solver:
+    """Convenience owner of one handle for torch tensors (marshalling only)."""
+
+    def __init__(self, H, W, sides, c_table, variant="standard", batch=1, schedule=SMRE_SCHED_AUTO):
+        v = {"standard": SMRE_STANDARD, "incomplete": SMRE_INCOMPLETE}.get(variant, variant)
+        self.H, self.W, self.batch, self.variant = int(H), int(W), int(batch), v
+        self.handle = smre_create(H, W, batch, sides, c_table, v)
+        if schedule != SMRE_SCHED_AUTO:
+            smre_set_schedule(self.handle, schedule)
+
+    def project(self, y, n_sweeps, out=None, stream=None):
+        import torch
+        if not (y.is_cuda and y.dtype == torch.float32 and y.is_contiguous()):
+            raise ValueError("y must be a contiguous float32 CUDA tensor")
+        if y.numel() != self.batch * self.H * self.W:
+            raise ValueError("y has the wrong number of elements")
+        if out is None:
+            out = torch.empty_like(y)
+        elif not (out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+                  and out.numel() == y.numel()):
+            raise ValueError("out must be a contiguous float32 CUDA tensor of y's size")
+        st = torch.cuda.current_stream(y.device) if stream is None else stream
+        smre_project(self.handle, y.data_ptr(), out.data_ptr(), n_sweeps, st.cuda_stream)
+        return out
+
+    def project_host(self, y_np, n_sweeps, out=None, stream=0):
+        y_np = np.ascontiguousarray(y_np, dtype=np.float32)
+        if y_np.size != self.batch * self.H * self.W:
+            raise ValueError("y has the wrong number of elements")
+        if out is None:
+            out = np.empty_like(y_np)
+        smre_project_host(self.handle, y_np.ctypes.data, out.ctypes.data, n_sweeps, stream)
+        return out
+
+    def increments(self):
+        import torch
+        F, _, _ = smre_info(self.handle)
+        q = torch.empty((F, self.batch, self.H, self.W), dtype=torch.float32, device="cuda")
+        smre_export_increments(self.handle, q.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        return q
+
+    info = property(lambda self: smre_info(self.handle))
+    last_launch = property(lambda self: smre_last_launch(self.handle))
+
+    def families(self):
+        return [smre_family(self.handle, i) for i in range(self.info[0])]
+
+    def close(self):
+        if self.handle:
+            smre_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,163 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element,
+on the five BASELINE.json configs at full size and on small / ragged / degenerate cases."""
+import numpy as np
+import pytest
+
+import smre_inputs as si
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+import paper_1503_03492_b200 as smre  # noqa: E402
+
+SCHEDULES = {"graph": smre.SMRE_SCHED_GRAPH, "persistent": smre.SMRE_SCHED_PERSISTENT}
+
+
+def gpu_project(y, sides, c, variant, n_sweeps, schedule=smre.SMRE_SCHED_AUTO, in_place=False):
+    y = np.ascontiguousarray(y, dtype=np.float32)
+    batch = 1 if y.ndim == 2 else y.shape[0]
+    sol = smre.Solver(y.shape[-2], y.shape[-1], sides, c, variant, batch, schedule)
+    try:
+        yt = torch.from_numpy(y).cuda()
+        out = sol.project(yt, n_sweeps, out=yt if in_place else None)
+        torch.cuda.synchronize()
+        return out.cpu().numpy(), sol.last_launch
+    finally:
+        sol.close()
+
+
+# ---- the five configs, full size, in the launch configuration bench.py times -------------------
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
+def test_config_full_size(oracle, idx):
+    w = si.config(idx)
+    x_gpu, launch = gpu_project(w.y, w.sides, w.c, w.variant, w.n_sweeps)
+    x_ref = oracle.project(w.y, w.sides, w.c, w.n_sweeps, w.variant)
+    d = parity.compare(oracle, w.y, x_gpu, x_ref, w.sides, w.c, w.variant)
+    print(f"\n{w.name}: {d} launch={launch}")
+    assert d["violated"] + d["in_band"] > 0          # finite sweeps: the comparison is not vacuous
+    assert launch[1] > 0
+
+
+# ---- every scheduler of the standard variant gives the same bits -------------------------------
+@pytest.mark.parametrize("idx,n", [(0, 50), (1, 3)])
+def test_schedulers_agree_bitwise(idx, n):
+    w = si.config(idx)
+    res = {}
+    for name, sch in SCHEDULES.items():
+        try:
+            res[name], launch = gpu_project(w.y, w.sides, w.c, "standard", n, sch)
+            assert launch[0] == sch
+        except smre.SmreError as e:
+            assert e.status == smre.smre.SMRE_EUNSUPPORTED
+    assert "graph" in res
+    for name, x in res.items():
+        assert np.array_equal(x, res["graph"]), name
+
+
+# ---- small, ragged, degenerate --------------------------------------------------------------------
+CASES = [
+    # H, W, batch, sides, variant, sweeps
+    (37, 53, 1, [1, 2, 3, 4, 5], "standard", 7),          # ragged: nothing divides
+    (64, 40, 3, [3, 1, 6], "standard", 5),                # batch > 1, sides not ascending
+    (33, 35, 1, [7, 8], "standard", 9),
+    (40, 72, 2, [16, 5], "standard", 4),
+    (70, 66, 1, [32, 17, 2], "standard", 3),              # largest compiled side
+    (8, 8, 1, [8], "standard", 3),                        # one window = the image
+    (5, 7, 1, [1], "standard", 2),                        # clip only
+    (50, 61, 1, [1, 2, 4, 8], "incomplete", 11),          # ragged ICD, K = 3
+    (64, 64, 5, [1, 2, 3, 4, 5, 6, 7, 8], "incomplete", 20),
+    (45, 99, 2, [1, 2, 4, 8, 16], "incomplete", 6),       # K = 4
+    (70, 83, 2, [1, 2, 4, 8, 16, 32], "incomplete", 5),   # K = 5, the paper's own depth
+    (19, 23, 1, [1, 2, 4], "incomplete", 8),              # K = 2
+    (9, 11, 3, [1, 2], "incomplete", 4),                  # K = 1
+    (6, 5, 1, [1], "incomplete", 3),                      # K = 0
+    (16, 16, 1, [1, 2, 4, 8, 16], "incomplete", 9),       # image = one tile
+]
+
+
+@pytest.mark.parametrize("H,W,B,sides,variant,n", CASES)
+def test_small_and_ragged(oracle, H, W, B, sides, variant, n):
+    rng = np.random.default_rng(H * 1000 + W)
+    y = (1.6 * rng.standard_normal((B, H, W))).astype(np.float32)
+    y[:, : H // 2, : W // 2] += 1.5
+    if B == 1:
+        y = y[0]
+    c = si.thresholds(sides)
+    x_ref = oracle.project(y, sides, c, n, variant)
+    scheds = list(SCHEDULES.values()) if variant == "standard" else [smre.SMRE_SCHED_AUTO]
+    ran = 0
+    for sch in scheds:
+        try:
+            x_gpu, _ = gpu_project(y, sides, c, variant, n, sch)
+        except smre.SmreError as e:
+            assert e.status == smre.smre.SMRE_EUNSUPPORTED and sch == smre.SMRE_SCHED_PERSISTENT
+            continue
+        ran += 1
+        d = parity.compare(oracle, y, x_gpu, x_ref, sides, c, variant)
+        assert np.abs(x_ref - y).max() > 0.05, "vacuous case"
+        assert d["max_abs_err"] < 2e-5
+    assert ran >= 1
+
+
+def test_in_place_and_identity_on_feasible_input(oracle):
+    rng = np.random.default_rng(5)
+    sides = np.arange(1, 9)
+    c = si.thresholds(sides)
+    y = (0.2 * rng.standard_normal((48, 52))).astype(np.float32)       # feasible: P2
+    for variant in ("standard", "incomplete"):
+        x, _ = gpu_project(y, sides, c, variant, 3)
+        assert np.array_equal(x, y)
+    w = si.config(0)
+    for variant in ("standard", "incomplete"):
+        a, _ = gpu_project(w.y, [1, 2, 4], si.thresholds([1, 2, 4]), variant, 6)
+        b, _ = gpu_project(w.y, [1, 2, 4], si.thresholds([1, 2, 4]), variant, 6, in_place=True)
+        assert np.array_equal(a, b)
+
+
+def test_exported_increments_and_host_path(oracle):
+    w = si.config(0)
+    sol = smre.Solver(w.H, w.W, w.sides, w.c, "standard")
+    yt = torch.from_numpy(w.y).cuda()
+    x = sol.project(yt, 20)
+    q = sol.increments()
+    torch.cuda.synchronize()
+    x_ref, q_ref = oracle.project_std(w.y, w.sides, w.c, 20, return_q=True)
+    assert sol.info == (30, 15630, 30 * 64 * 64 * 4)
+    fams = oracle.std_family_list(w.sides, w.c)
+    for i, f in enumerate(sol.families()):
+        assert f[:3] == fams[i][:3] and abs(f[3] - fams[i][3]) < 1e-6
+    qn = q.cpu().numpy()[:, 0].astype(np.float64)
+    # conservation x + sum_f q_f == y (P5) holds on the GPU too, up to fp32 rounding
+    assert np.abs(x.cpu().numpy() + qn.sum(0) - w.y).max() < 2e-5
+    assert np.abs(qn - q_ref).max() < 2e-5
+    # same windows carry a multiplier, away from the decision boundary
+    big = np.abs(q_ref) > 1e-4
+    assert np.array_equal(np.abs(qn) > 0, np.abs(q_ref) > 0) or (np.abs(qn)[big] > 0).all()
+    # a second call starts from q = 0 again (no state carried between calls)
+    x2 = sol.project(yt, 20)
+    assert torch.equal(x, x2)
+    xh = sol.project_host(w.y, 20)
+    assert np.array_equal(xh, x.cpu().numpy())
+    sol.close()
+
+
+def test_error_codes_on_device():
+    sol = smre.Solver(16, 16, [1, 2], si.thresholds([1, 2]), "standard")
+    yt = torch.zeros(16, 16, device="cuda")
+    with pytest.raises(smre.SmreError) as e:
+        smre.smre_project(sol.handle, yt.data_ptr(), yt.data_ptr(), 0, 0)
+    assert e.value.status == smre.smre.SMRE_EINVAL
+    with pytest.raises(smre.SmreError):
+        smre.smre_project(sol.handle, None, yt.data_ptr(), 1, 0)
+    with pytest.raises(smre.SmreError):
+        smre.smre_family(sol.handle, 99)
+    sol.close()
+    with pytest.raises(smre.SmreError) as e:
+        smre.Solver(16, 16, [1, 2, 8], si.thresholds([1, 2, 8]), "incomplete")   # level 4 missing
+    assert e.value.status == smre.smre.SMRE_EINVAL
+    icd = smre.Solver(16, 16, [1, 2], si.thresholds([1, 2]), "incomplete")
+    assert icd.info[0] == 3 and icd.info[2] == 0
+    with pytest.raises(smre.SmreError):
+        icd.increments()
+    icd.close()
