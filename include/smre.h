@@ -119,7 +119,9 @@ smre_status smre_family(smre_handle h, int idx, int *side, int *oy, int *ox, flo
 smre_status smre_export_increments(smre_handle h, float *q_out_dev, void *cuda_stream);
 
 /* Scheduler actually used by the last smre_project (smre_schedule value), number of kernels it
- * launched, and the persistent schedule's tile grid (0 x 0 if unused).  Pointers may be NULL. */
+ * launched, and the persistent schedule's tile grid (0 x 0 if unused).  Pointers may be NULL.
+ * After a persistent run this call SYNCHRONISES with the device to read the scheduler's health flag
+ * and returns SMRE_ECUDA if a neighbour hand-off timed out (the result is then invalid). */
 smre_status smre_last_launch(smre_handle h, int *schedule_used, long long *kernel_launches,
                              int *tiles_y, int *tiles_x);
 

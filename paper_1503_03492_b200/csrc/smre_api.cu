@@ -284,7 +284,11 @@ extern "C" smre_status smre_last_launch(smre_handle h, int *schedule_used, long 
     if (schedule_used) *schedule_used = h->last_schedule;
     if (kernel_launches) *kernel_launches = h->last_launches;
     int ty = 0, tx = 0;
-    if (h->plan && h->last_schedule == SMRE_SCHED_PERSISTENT) persistent_plan_tiles(h->plan, &ty, &tx);
+    if (h->plan && h->last_schedule == SMRE_SCHED_PERSISTENT) {
+        persistent_plan_tiles(h->plan, &ty, &tx);
+        if (persistent_plan_status(h->plan) != 0)
+            return fail(SMRE_ECUDA, "persistent scheduler: a neighbour hand-off timed out (result invalid)");
+    }
     if (tiles_y) *tiles_y = ty;
     if (tiles_x) *tiles_x = tx;
     return SMRE_OK;

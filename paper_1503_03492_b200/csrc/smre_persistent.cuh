@@ -13,6 +13,8 @@ PersistentPlan *persistent_plan_create(int H, int W, int B, const std::vector<Fa
                                        float *q, float *xwork);
 void persistent_plan_destroy(PersistentPlan *p);
 void persistent_plan_tiles(const PersistentPlan *p, int *tiles_y, int *tiles_x);
+// 0 = healthy, 1 = a mailbox poll timed out in some launch (protocol failure), -1 = cannot read.  Synchronises.
+int persistent_plan_status(const PersistentPlan *p);
 
 // Whole projection: x <- y, q <- 0, n_sweeps ordered sweeps, x_out <- x.  Asynchronous on st.
 cudaError_t persistent_run(PersistentPlan *p, const float *y, float *x_out, int n_sweeps,
