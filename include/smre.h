@@ -56,8 +56,9 @@ typedef enum { SMRE_STANDARD = 0, SMRE_INCOMPLETE = 1 } smre_variant;
 typedef enum {
     SMRE_SCHED_AUTO = 0,        /* persistent if the image tiles fit on chip, else graph */
     SMRE_SCHED_GRAPH = 1,       /* one kernel per family, one captured CUDA graph per sweep */
-    SMRE_SCHED_PERSISTENT = 2   /* one cooperative kernel per call: x tiles resident in shared
-                                   memory, q streamed from HBM, neighbour hand-off between CTAs */
+    SMRE_SCHED_PERSISTENT = 2   /* "conveyor": one cooperative kernel per call; x tiles resident in
+                                   shared memory, tile boundaries that follow each family's window
+                                   grid, one-directional hand-off between CTAs, q streamed from HBM */
 } smre_schedule;
 
 #define SMRE_MAX_SIDE 32        /* largest window side (the paper's L_SMRE = 32) */
@@ -124,6 +125,15 @@ smre_status smre_export_increments(smre_handle h, float *q_out_dev, void *cuda_s
  * and returns SMRE_ECUDA if a neighbour hand-off timed out (the result is then invalid). */
 smre_status smre_last_launch(smre_handle h, int *schedule_used, long long *kernel_launches,
                              int *tiles_y, int *tiles_x);
+
+/* Host-only planning check of the conveyor schedule (no device needed, nothing allocated): plans
+ * the moving tile boundaries for n_sweeps sweeps of the standard variant over sides[] on an H x W
+ * image with at most max_ctas tiles, verifies every hand-off invariant of the plan, and reports the
+ * tile grid, the largest tile and the size of the boundary tables.  SMRE_EUNSUPPORTED (with the
+ * reason in smre_last_error) if the conveyor cannot tile the problem.  Out pointers may be NULL. */
+smre_status smre_plan_check(int H, int W, const int *sides, int n_sides, int n_sweeps, int max_ctas,
+                            int *tiles_y, int *tiles_x, int *max_tile_h, int *max_tile_w,
+                            long long *table_bytes);
 
 /* Text of the last error on the calling thread ("" if none).  Never NULL. */
 const char *smre_last_error(void);

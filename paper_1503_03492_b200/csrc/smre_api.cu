@@ -1,9 +1,9 @@
 // C ABI of include/smre.h: handle, argument validation, family enumeration and the two sweep
 // schedulers' host side.  Every step of the path runs in the kernels of smre_family.cu,
-// smre_persistent.cu and smre_icd.cu; there is no CPU path.
+// smre_conveyor.cu and smre_icd.cu; there is no CPU path.
 #include "../../include/smre.h"
 #include "smre_common.cuh"
-#include "smre_persistent.cuh"
+#include "smre_conveyor.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -39,6 +39,7 @@ static smre_status cuda_fail(cudaError_t e, const char *what)
 
 struct smre_handle_s {
     int H = 0, W = 0, B = 0;
+    int Wq = 0;                        // row pitch of the q planes: W rounded up to a multiple of 4
     smre_variant variant = SMRE_STANDARD;
     std::vector<int> sides;
     std::vector<float> c;
@@ -46,12 +47,12 @@ struct smre_handle_s {
     std::vector<int> pass_shift;       // incomplete: shift index of each level pass
     long long windows_per_sweep = 0;
     // standard
-    float *q = nullptr;                // [F][B][H][W]
+    float *q = nullptr;                // [F][B][H][Wq]
     float *xwork = nullptr;            // [B][H][W]
     size_t q_bytes = 0;
     smre_schedule schedule = SMRE_SCHED_AUTO;
     cudaGraphExec_t sweep_graph = nullptr;
-    PersistentPlan *plan = nullptr;    // null if the image cannot be held on chip
+    ConveyorPlan *plan = nullptr;      // null if the conveyor cannot tile this problem
     // incomplete
     int K = 0;
     IcdLevels levels{};
@@ -70,9 +71,9 @@ static smre_status build_sweep_graph(smre_handle h)
     CU(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
     cudaGraph_t g = nullptr;
     cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
-    const size_t plane = (size_t)h->B * h->H * h->W;
+    const size_t plane = (size_t)h->B * h->H * h->Wq;
     for (size_t f = 0; e == cudaSuccess && f < h->fams.size(); ++f)
-        e = launch_family_pass(h->xwork, h->q + f * plane, h->B, h->H, h->W, h->fams[f], cs);
+        e = launch_family_pass(h->xwork, h->q + f * plane, h->B, h->H, h->W, h->Wq, h->fams[f], cs);
     cudaError_t e2 = cudaStreamEndCapture(cs, &g);
     if (e == cudaSuccess) e = e2;
     if (e == cudaSuccess) e = cudaGraphInstantiate(&h->sweep_graph, g, 0);
@@ -113,7 +114,7 @@ extern "C" smre_status smre_create(smre_handle *out, int H, int W, int batch, co
 
     smre_handle h = new (std::nothrow) smre_handle_s;
     if (!h) return fail(SMRE_ENOMEM, "host allocation failed");
-    h->H = H; h->W = W; h->B = batch; h->variant = variant;
+    h->H = H; h->W = W; h->Wq = (W + 3) & ~3; h->B = batch; h->variant = variant;
     h->sides.assign(sides, sides + n_sides);
     h->c.assign(c_table, c_table + n_sides);
 
@@ -128,13 +129,13 @@ extern "C" smre_status smre_create(smre_handle *out, int H, int W, int batch, co
                     h->windows_per_sweep += (long long)f.ny * f.nx * batch;
                 }
         const size_t plane = (size_t)batch * H * W * sizeof(float);
-        h->q_bytes = plane * h->fams.size();
+        h->q_bytes = (size_t)batch * H * h->Wq * sizeof(float) * h->fams.size();
         cudaError_t e = cudaMalloc(&h->q, h->q_bytes);
         if (e == cudaSuccess) e = cudaMalloc(&h->xwork, plane);
         if (e != cudaSuccess) { smre_status s = cuda_fail(e, "allocating increment planes"); smre_destroy(h); return s; }
         smre_status s = build_sweep_graph(h);
         if (s != SMRE_OK) { smre_destroy(h); return s; }
-        h->plan = persistent_plan_create(H, W, batch, h->fams, h->q, h->xwork);   // may be null
+        h->plan = conveyor_plan_create(H, W, batch, h->fams, h->q, h->xwork);     // may be null
     } else {
         int K = 0;
         while ((2 << K) <= smax) ++K;
@@ -166,7 +167,7 @@ extern "C" smre_status smre_create(smre_handle *out, int H, int W, int batch, co
 extern "C" smre_status smre_destroy(smre_handle h)
 {
     if (!h) return SMRE_OK;
-    if (h->plan) persistent_plan_destroy(h->plan);
+    if (h->plan) conveyor_plan_destroy(h->plan);
     if (h->sweep_graph) cudaGraphExecDestroy(h->sweep_graph);
     if (h->q) cudaFree(h->q);
     if (h->xwork) cudaFree(h->xwork);
@@ -212,9 +213,12 @@ extern "C" smre_status smre_project(smre_handle h, const float *y_dev, float *x_
     const bool persistent = h->plan && (h->schedule == SMRE_SCHED_PERSISTENT ||
                                         h->schedule == SMRE_SCHED_AUTO);
     if (persistent) {
-        h->last_schedule = SMRE_SCHED_PERSISTENT;
-        CU(persistent_run(h->plan, y_dev, x_out_dev, n_sweeps, st, &h->last_launches));
-        return SMRE_OK;
+        cudaError_t e = conveyor_run(h->plan, y_dev, x_out_dev, n_sweeps, st, &h->last_launches);
+        if (e == cudaSuccess) { h->last_schedule = SMRE_SCHED_PERSISTENT; return SMRE_OK; }
+        if (e != cudaErrorNotSupported) return cuda_fail(e, "conveyor_run");
+        if (h->schedule == SMRE_SCHED_PERSISTENT)
+            return fail(SMRE_EUNSUPPORTED, "the conveyor cannot tile %d sweeps of this problem", n_sweeps);
+        h->last_launches = 0;                      // SMRE_SCHED_AUTO: fall through to the graph schedule
     }
     // graph schedule: x <- y, q <- 0 (Alg. 2: q_{0,s} = 0), then n_sweeps replays of the sweep graph
     h->last_schedule = SMRE_SCHED_GRAPH;
@@ -251,7 +255,7 @@ extern "C" smre_status smre_info(smre_handle h, int *n_families, long long *wind
     if (!h) return fail(SMRE_EINVAL, "handle is NULL");
     if (n_families) *n_families = (int)h->fams.size();
     if (windows_per_sweep) *windows_per_sweep = h->windows_per_sweep;
-    if (increment_bytes) *increment_bytes = (long long)h->q_bytes;
+    if (increment_bytes) *increment_bytes = (long long)h->fams.size() * h->B * h->H * h->W * 4 * (h->q ? 1 : 0);
     return SMRE_OK;
 }
 
@@ -273,7 +277,35 @@ extern "C" smre_status smre_export_increments(smre_handle h, float *q_out_dev, v
     if (!q_out_dev) return fail(SMRE_EINVAL, "q_out_dev is NULL");
     if (h->variant != SMRE_STANDARD)
         return fail(SMRE_EUNSUPPORTED, "the incomplete variant keeps no increments in device memory");
-    CU(cudaMemcpyAsync(q_out_dev, h->q, h->q_bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    CU(cudaMemcpy2DAsync(q_out_dev, (size_t)h->W * 4, h->q, (size_t)h->Wq * 4, (size_t)h->W * 4,
+                         h->fams.size() * (size_t)h->B * h->H, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    return SMRE_OK;
+}
+
+extern "C" smre_status smre_plan_check(int H, int W, const int *sides, int n_sides, int n_sweeps,
+                                       int max_ctas, int *tiles_y, int *tiles_x, int *max_tile_h,
+                                       int *max_tile_w, long long *table_bytes)
+{
+    g_err[0] = 0;
+    if (!sides || H <= 0 || W <= 0 || n_sides <= 0 || n_sweeps <= 0 || max_ctas <= 0)
+        return fail(SMRE_EINVAL, "smre_plan_check: bad argument");
+    std::vector<Family> fams;
+    for (int a = 0; a < n_sides; ++a) {
+        if (sides[a] < 1 || sides[a] > H || sides[a] > W || sides[a] > SMRE_MAX_SIDE)
+            return fail(SMRE_EINVAL, "side %d outside [1, min(H, W, SMRE_MAX_SIDE)]", sides[a]);
+        for (int oy = 0; oy < sides[a]; ++oy)
+            for (int ox = 0; ox < sides[a]; ++ox)
+                fams.push_back(Family{sides[a], oy, ox, (H - oy) / sides[a], (W - ox) / sides[a], 1.0f, 1.0f});
+    }
+    ConveyorSummary cs;
+    char why[200] = "";
+    if (!conveyor_summary(H, W, fams, n_sweeps, max_ctas, &cs, why, sizeof why))
+        return fail(SMRE_EUNSUPPORTED, "conveyor: %s", why);
+    if (tiles_y) *tiles_y = cs.tiles_y;
+    if (tiles_x) *tiles_x = cs.tiles_x;
+    if (max_tile_h) *max_tile_h = cs.max_h;
+    if (max_tile_w) *max_tile_w = cs.max_w;
+    if (table_bytes) *table_bytes = cs.table_bytes;
     return SMRE_OK;
 }
 
@@ -285,9 +317,9 @@ extern "C" smre_status smre_last_launch(smre_handle h, int *schedule_used, long 
     if (kernel_launches) *kernel_launches = h->last_launches;
     int ty = 0, tx = 0;
     if (h->plan && h->last_schedule == SMRE_SCHED_PERSISTENT) {
-        persistent_plan_tiles(h->plan, &ty, &tx);
-        if (persistent_plan_status(h->plan) != 0)
-            return fail(SMRE_ECUDA, "persistent scheduler: a neighbour hand-off timed out (result invalid)");
+        conveyor_plan_tiles(h->plan, &ty, &tx);
+        if (conveyor_plan_status(h->plan) != 0)
+            return fail(SMRE_ECUDA, "conveyor scheduler: a neighbour hand-off timed out (result invalid)");
     }
     if (tiles_y) *tiles_y = ty;
     if (tiles_x) *tiles_x = tx;

@@ -29,8 +29,9 @@ __device__ __forceinline__ float ball_scale(float n2, float c, float sqrt_c) {
 
 // ---- launchers implemented in the .cu files --------------------------------------------------
 
-// smre_family.cu: one family pass over all frames (schedule SMRE_SCHED_GRAPH).
-cudaError_t launch_family_pass(float *x, float *q_plane, int B, int H, int W, const Family &f,
+// smre_family.cu: one family pass over all frames (schedule SMRE_SCHED_GRAPH).  x: [B][H][W];
+// q_plane: [B][H][Wq], Wq = W rounded up to a multiple of 4 (16-byte aligned rows for cp.async).
+cudaError_t launch_family_pass(float *x, float *q_plane, int B, int H, int W, int Wq, const Family &f,
                                cudaStream_t st);
 
 // smre_icd.cu: one shift of the incomplete Dykstra (P_{Omega^i}).

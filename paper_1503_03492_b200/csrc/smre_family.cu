@@ -16,7 +16,7 @@ namespace smre {
 
 template <int G>
 __global__ void __launch_bounds__(256)
-family_pass_kernel(float *__restrict__ x, float *__restrict__ q, int H, int W, Family f,
+family_pass_kernel(float *__restrict__ x, float *__restrict__ q, int H, int W, int Wq, Family f,
                    int chunks_per_row)
 {
     constexpr int WPW = 32 / G;                      // windows per warp
@@ -30,6 +30,8 @@ family_pass_kernel(float *__restrict__ x, float *__restrict__ q, int H, int W, F
     const bool on = (wi < f.nx) && (j < f.side);
     const size_t base = ((size_t)blockIdx.y * H + (size_t)(f.oy + wrow * f.side)) * W
                       + (size_t)(f.ox + wi * f.side + j);
+    const size_t qbase = ((size_t)blockIdx.y * H + (size_t)(f.oy + wrow * f.side)) * Wq
+                       + (size_t)(f.ox + wi * f.side + j);     // q planes have row pitch Wq
 
     float v[G];
     float part = 0.0f;
@@ -37,8 +39,7 @@ family_pass_kernel(float *__restrict__ x, float *__restrict__ q, int H, int W, F
     for (int r = 0; r < G; ++r) {
         v[r] = 0.0f;
         if (r < f.side && on) {
-            const size_t i = base + (size_t)r * W;
-            v[r] = x[i] + q[i];
+            v[r] = x[base + (size_t)r * W] + q[qbase + (size_t)r * Wq];
         }
         part = fmaf(v[r], v[r], part);
     }
@@ -49,16 +50,15 @@ family_pass_kernel(float *__restrict__ x, float *__restrict__ q, int H, int W, F
 #pragma unroll
     for (int r = 0; r < G; ++r) {
         if (r < f.side && on) {
-            const size_t i = base + (size_t)r * W;
             const float xn = alpha * v[r];
-            x[i] = xn;
-            q[i] = v[r] - xn;
+            x[base + (size_t)r * W] = xn;
+            q[qbase + (size_t)r * Wq] = v[r] - xn;
         }
     }
 }
 
 template <int G>
-static cudaError_t launch_g(float *x, float *q, int B, int H, int W, const Family &f, cudaStream_t st)
+static cudaError_t launch_g(float *x, float *q, int B, int H, int W, int Wq, const Family &f, cudaStream_t st)
 {
     constexpr int WPW = 32 / G;
     const int chunks = (f.nx + WPW - 1) / WPW;
@@ -66,20 +66,20 @@ static cudaError_t launch_g(float *x, float *q, int B, int H, int W, const Famil
     if (warps == 0) return cudaSuccess;
     const int warps_per_block = 8;
     dim3 grid((unsigned)((warps + warps_per_block - 1) / warps_per_block), (unsigned)B);
-    family_pass_kernel<G><<<grid, warps_per_block * 32, 0, st>>>(x, q, H, W, f, chunks);
+    family_pass_kernel<G><<<grid, warps_per_block * 32, 0, st>>>(x, q, H, W, Wq, f, chunks);
     return cudaGetLastError();
 }
 
-cudaError_t launch_family_pass(float *x, float *q_plane, int B, int H, int W, const Family &f,
+cudaError_t launch_family_pass(float *x, float *q_plane, int B, int H, int W, int Wq, const Family &f,
                                cudaStream_t st)
 {
     const int s = f.side;
-    if (s <= 1) return launch_g<1>(x, q_plane, B, H, W, f, st);
-    if (s <= 2) return launch_g<2>(x, q_plane, B, H, W, f, st);
-    if (s <= 4) return launch_g<4>(x, q_plane, B, H, W, f, st);
-    if (s <= 8) return launch_g<8>(x, q_plane, B, H, W, f, st);
-    if (s <= 16) return launch_g<16>(x, q_plane, B, H, W, f, st);
-    return launch_g<32>(x, q_plane, B, H, W, f, st);
+    if (s <= 1) return launch_g<1>(x, q_plane, B, H, W, Wq, f, st);
+    if (s <= 2) return launch_g<2>(x, q_plane, B, H, W, Wq, f, st);
+    if (s <= 4) return launch_g<4>(x, q_plane, B, H, W, Wq, f, st);
+    if (s <= 8) return launch_g<8>(x, q_plane, B, H, W, Wq, f, st);
+    if (s <= 16) return launch_g<16>(x, q_plane, B, H, W, Wq, f, st);
+    return launch_g<32>(x, q_plane, B, H, W, Wq, f, st);
 }
 
 }  // namespace smre

@@ -21,6 +21,7 @@ _STATUS = {0: "SMRE_OK", 1: "SMRE_EINVAL", 2: "SMRE_EUNSUPPORTED", 3: "SMRE_ENOM
 exported_symbols = (
     "smre_create", "smre_project", "smre_project_host", "smre_destroy", "smre_set_schedule",
     "smre_info", "smre_family", "smre_export_increments", "smre_last_launch", "smre_last_error",
+    "smre_plan_check",
 )
 
 
@@ -58,6 +59,8 @@ def load_library(build_if_missing: bool = True):
     lib.smre_family.argtypes = [_vp, ctypes.c_int, _ip, _ip, _ip, _fp]
     lib.smre_export_increments.argtypes = [_vp, _vp, _vp]
     lib.smre_last_launch.argtypes = [_vp, _ip, _llp, _ip, _ip]
+    lib.smre_plan_check.argtypes = [ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                    _ip, _ip, _ip, _ip, _llp]
     for name in exported_symbols:
         getattr(lib, name).restype = ctypes.c_int
     lib.smre_last_error.restype = ctypes.c_char_p
@@ -129,6 +132,17 @@ def smre_last_launch(handle):
     _check(load_library().smre_last_launch(handle, ctypes.byref(s), ctypes.byref(n),
                                            ctypes.byref(ty), ctypes.byref(tx)))
     return s.value, n.value, ty.value, tx.value
+
+
+def smre_plan_check(H, W, sides, n_sweeps, max_ctas=148):
+    """Host-only: -> (tiles_y, tiles_x, max_tile_h, max_tile_w, table_bytes) of the conveyor plan."""
+    sides = np.ascontiguousarray(sides, dtype=np.int32)
+    ty, tx, mh, mw, tb = (ctypes.c_int(), ctypes.c_int(), ctypes.c_int(), ctypes.c_int(),
+                          ctypes.c_longlong())
+    _check(load_library().smre_plan_check(int(H), int(W), sides.ctypes.data_as(_ip), len(sides),
+                                          int(n_sweeps), int(max_ctas), ctypes.byref(ty), ctypes.byref(tx),
+                                          ctypes.byref(mh), ctypes.byref(mw), ctypes.byref(tb)))
+    return ty.value, tx.value, mh.value, mw.value, tb.value
 
 
 class Solver:
