@@ -43,8 +43,9 @@ struct CParams {
     const AxisEntry *taby;        // [total][NR]
     const AxisEntry *tabx;        // [total][NC]
     unsigned long long *mbox;     // [n_cta][CV_D][CV_MBW] words {tag:32 | value:32}
-    unsigned *prog;               // [n_cta] "mailbox read up to and including step"
+    unsigned *prog;               // [n_cta][CV_PROG_STRIDE] "mailbox read up to and including step" (one line each)
     int *status;                  // != 0: a poll timed out somewhere (protocol bug) -> everybody leaves
+    unsigned long long *trace;    // debug (SMRE_CV_TRACE): [n_cta][total][8] globaltimer stamps, or null
     int F, total;
     int H, W, Wq, B_total, frame0;   // Wq: row pitch of the q planes (W rounded up to 4)
     int NR, NC;
@@ -82,6 +83,7 @@ __device__ __noinline__ unsigned long long poll_tag(const unsigned long long *p,
     for (unsigned spins = 1;; ++spins) {
         v = ld_u64_gpu(p);
         if ((unsigned)(v >> 32) == tag) break;
+        __nanosleep(64);                                   // polling a line bounces it between the L2 halves
         if ((spins & 63u) == 0) {
             if (*(volatile int *)status != 0) break;
             if (clock64() - t0 > 2000000000LL) { atomicExch(status, 1); break; }
@@ -95,6 +97,7 @@ __device__ __noinline__ unsigned poll_prog(const unsigned *p, unsigned need, int
     for (unsigned spins = 1;; ++spins) {
         v = ld_u32_gpu(p);
         if (v >= need) break;
+        __nanosleep(200);
         if ((spins & 63u) == 0) {
             if (*(volatile int *)status != 0) return need;
             if (clock64() - t0 > 2000000000LL) { atomicExch(status, 1); return need; }
@@ -112,70 +115,113 @@ __device__ __forceinline__ int mbox_col_word(int r, int c) { return ((c & (CV_SD
 __device__ __forceinline__ int mbox_row_word(int r, int c) { return CV_SD * 64 + (((r & (CV_SD - 1)) << 6) | (c & 63)); }
 
 struct Smem {
-    float xs[CV_PW * CV_PW];                 // the x tile, torus addressed
-    float qs[CV_NST][CV_PW * CV_PW];         // q stages, same addressing
+    float xs[CV_PW * CV_PW];                 // the x tile, torus addressed by image (row, column)
+    float qs[CV_NST][CV_PW * CV_PW];         // q stages: [(row - first window row) * 64 + (column - c0)]
     AxisEntry tab[CV_TR][2];                 // [step % CV_TR][0 = y, 1 = x]
     CFamily fams[CV_MAX_F];
-    unsigned nbr_prog[4];                    // cached progress of the left / up / up-left CTAs
 };
 
-// Arrival i of the step described by (ey, ex): pixel and mailbox word.  Column strip first
-// (all tile rows x columns [ex.A, ex.R)), then the row strip (rows [ey.A, ey.R) x columns [ex.L, ex.A)).
-__device__ __forceinline__ void arrival(const AxisEntry &ey, const AxisEntry &ex, int i, int n_col,
-                                        int &r, int &c, int &word) {
-    const int h = ey.R - ey.L;
-    if (i < n_col) {
-        const int k = i / h;
-        c = ex.A + k; r = ey.L + (i - k * h);
-        word = mbox_col_word(r, c);
-    } else {
-        const int w = ex.A - ex.L, j = i - n_col;
-        const int k = j / w;
-        r = ey.A + k; c = ex.L + (j - k * w);
-        word = mbox_row_word(r, c);
+// The windows of one step inside this CTA's tile, for a compile-time window edge S.
+// G = lanes per window (power of two >= S): lane j of a window owns column j.  A lane handles KR
+// vertically stacked windows (S * KR rows of its column) so that the per-item index arithmetic is
+// paid once per ~8 pixels whatever the window size.  Summation order per window = family_pass_kernel's:
+// rows top to bottom inside the lane (fma), then an xor-shuffle tree over the G lanes.
+template <int S, int KR>
+__device__ __forceinline__ void project_tile(Smem &sm, const float *qst, float *__restrict__ qplane,
+                                             const AxisEntry &ey, const AxisEntry &ex, float c, float sqrt_c,
+                                             int Wq, bool first_sweep, int cw, int lane)
+{
+    constexpr int G = S <= 1 ? 1 : S <= 2 ? 2 : S <= 4 ? 4 : 8;
+    constexpr int R = S * KR;
+    const int nwy = ey.nw, nwx = ex.nw;
+    const int nby = (nwy + KR - 1) / KR;                 // blocks of KR window rows
+    const int n_items = nby * nwx * G;
+    const int c0 = ex.w0 & ~3;
+    for (int base = cw * 32; base < n_items; base += CV_NCW * 32) {
+        const int item = base + lane;
+        const int grp = item / G, j = item % G;
+        const int by = (int)(((unsigned)grp * ex.magic) >> 20), wix = grp - by * nwx;
+        const bool on = item < n_items && j < S;
+        const int nwin = on ? min(KR, nwy - by * KR) : 0;    // valid windows of this block
+        const int rr0 = by * R;
+        const int r0 = ey.w0 + rr0, cc = ex.w0 + wix * S + j;
+        const int xi0 = tidx(r0, cc);
+        const float *qs0 = qst + rr0 * CV_PW + (cc - c0);
+        float *qg = qplane + (size_t)r0 * Wq + cc;
+        float v[R], part[KR];
+#pragma unroll
+        for (int k = 0; k < KR; ++k) {
+            part[k] = 0.0f;
+#pragma unroll
+            for (int r = 0; r < S; ++r) {
+                const int rr = k * S + r;
+                v[rr] = 0.0f;
+                if (k < nwin) {
+                    const float xv = sm.xs[(xi0 + rr * CV_PW) & (CV_PW * CV_PW - 1)];
+                    v[rr] = first_sweep ? xv : xv + qs0[rr * CV_PW];
+                }
+                part[k] = fmaf(v[rr], v[rr], part[k]);
+            }
+        }
+#pragma unroll
+        for (int m = G / 2; m > 0; m >>= 1)
+#pragma unroll
+            for (int k = 0; k < KR; ++k) part[k] += __shfl_xor_sync(0xffffffffu, part[k], m);
+#pragma unroll
+        for (int k = 0; k < KR; ++k) {
+            const float alpha = ball_scale(part[k], c, sqrt_c);
+#pragma unroll
+            for (int r = 0; r < S; ++r) {
+                const int rr = k * S + r;
+                if (k < nwin) {
+                    const float xn = alpha * v[rr];
+                    sm.xs[(xi0 + rr * CV_PW) & (CV_PW * CV_PW - 1)] = xn;
+                    __stcs(qg + (size_t)rr * Wq, v[rr] - xn);
+                }
+            }
+        }
     }
 }
 
-// The windows of one step inside this CTA's tile.  G = lanes per window (power of two >= side); lane j
-// of a window owns column j and keeps the `side` values of that column in registers.
+// Window edges above 8: G = 16 or 32 lanes per window, run-time edge s, one window per lane group.
 template <int G>
-__device__ __forceinline__ void project_tile(Smem &sm, const float *qst, float *__restrict__ qplane,
-                                             const AxisEntry &ey, const AxisEntry &ex, const CFamily &fam,
-                                             int W, bool first_sweep)
+__device__ __forceinline__ void project_tile_big(Smem &sm, const float *qst, float *__restrict__ qplane,
+                                                 const AxisEntry &ey, const AxisEntry &ex, int s, float c,
+                                                 float sqrt_c, int Wq, bool first_sweep, int cw, int lane)
 {
-    const int s = fam.side;
     const int nwx = ex.nw;
     const int n_items = ey.nw * nwx * G;
-    for (int base = 0; base < n_items; base += CV_NT) {
-        if (base + (int)(threadIdx.x & ~31u) >= n_items) break;        // warp-uniform: nothing left
-        const int item = base + threadIdx.x;
+    const int c0 = ex.w0 & ~3;
+    for (int base = cw * 32; base < n_items; base += CV_NCW * 32) {
+        const int item = base + lane;
         const int win = item / G, j = item % G;
         const int wiy = (int)(((unsigned)win * ex.magic) >> 20), wix = win - wiy * nwx;
         const bool on = item < n_items && j < s;
-        const int r0 = ey.w0 + wiy * s, c = ex.w0 + wix * s + j;
-        const int i0 = tidx(r0, c);
-        float *qg = qplane + (size_t)r0 * W + c;
+        const int rr0 = wiy * s;
+        const int r0 = ey.w0 + rr0, cc = ex.w0 + wix * s + j;
+        const int xi0 = tidx(r0, cc);
+        const float *qs0 = qst + rr0 * CV_PW + (cc - c0);
+        float *qg = qplane + (size_t)r0 * Wq + cc;
         float v[G];
         float part = 0.0f;
 #pragma unroll
         for (int r = 0; r < G; ++r) {
             v[r] = 0.0f;
             if (r < s && on) {
-                const int i = (i0 + (r << 6)) & (CV_PW * CV_PW - 1);
-                v[r] = sm.xs[i] + (first_sweep ? 0.0f : qst[i]);
+                const float xv = sm.xs[(xi0 + r * CV_PW) & (CV_PW * CV_PW - 1)];
+                v[r] = first_sweep ? xv : xv + qs0[r * CV_PW];
             }
             part = fmaf(v[r], v[r], part);
         }
 #pragma unroll
         for (int m = G / 2; m > 0; m >>= 1) part += __shfl_xor_sync(0xffffffffu, part, m);
-        const float alpha = ball_scale(part, fam.c, fam.sqrt_c);
+        const float alpha = ball_scale(part, c, sqrt_c);
 #pragma unroll
         for (int r = 0; r < G; ++r) {
             if (r < s && on) {
-                const int i = (i0 + (r << 6)) & (CV_PW * CV_PW - 1);
                 const float xn = alpha * v[r];
-                sm.xs[i] = xn;
-                __stcs(qg + (size_t)r * W, v[r] - xn);
+                sm.xs[(xi0 + r * CV_PW) & (CV_PW * CV_PW - 1)] = xn;
+                __stcs(qg + (size_t)r * Wq, v[r] - xn);
             }
         }
     }
@@ -186,7 +232,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Smem &sm = *reinterpret_cast<Smem *>(smem_raw);
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int cta = blockIdx.x;
     const int bl = cta / (p.NR * p.NC);
     const int t2 = cta - bl * p.NR * p.NC;
@@ -208,7 +254,6 @@ conveyor_kernel(const __grid_constant__ CParams p)
         const int g = i >> 1, ax = i & 1;
         sm.tab[g % CV_TR][ax] = ax ? p.tabx[(size_t)g * p.NC + cj] : p.taby[(size_t)g * p.NR + ci];
     }
-    if (tid < 4) sm.nbr_prog[tid] = 0;
     __syncthreads();
     {
         const AxisEntry ey = sm.tab[0][0], ex = sm.tab[0][1];
@@ -220,127 +265,157 @@ conveyor_kernel(const __grid_constant__ CParams p)
     }
     __syncthreads();
 
-    unsigned long long pend = 0;      // mailbox word loaded ahead of time (arrival index NT-1-tid)
-    unsigned prog_pend = 0;           // neighbour progress loaded ahead of time (tid 1..3)
-    int status_pend = 0;              // status flag loaded ahead of time (tid 0)
-    int f = 0;                        // family of step g
-    int fp = CV_PF % p.F;             // family of step g + CV_PF
-    const int hi = CV_NT - 1 - tid;   // hand-off duties go to the highest threads first
+    // role state (each used by one warp only)
+    unsigned long long pend0 = 0, pend1 = 0;   // receiver: mailbox words loaded one step ahead
+    unsigned prog_pend = 0, prog_seen = 0;     // sender lanes 1..3: progress of the receiving CTAs
+    int prog_iter = -1;                        // step at which prog_pend was requested (-1: none in flight)
+    int status_pend = 0;                       // receiver lane 0: the failure flag, loaded one step ahead
+    int f = 0;                                 // family of step g
+    int fp = CV_PF % p.F;                      // family of step g + CV_PF
 
     for (int g = 0; g < total; ++g) {
-        const AxisEntry ey = sm.tab[g % CV_TR][0], ex = sm.tab[g % CV_TR][1];
-        const CFamily fam = sm.fams[f];
-
-        // ---- (f) departures of step g-1 -> the neighbours' mailboxes, tagged g -----------------------
-        if (g > 0) {
-            const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
-            const int h = py.R - py.L, w = px.R - px.L;
-            const int n_col = h * (px.D - px.L);                    // columns [L, D), all rows
-            const int n_row = (py.D - py.L) * (px.R - px.D);         // rows [L, D), columns [D, R)
-            const int n_dep = n_col + n_row;
-            (void)w;
-            for (int i = hi; i < n_dep; i += CV_NT) {
-                int r, c, word;
-                if (i < n_col) {
-                    const int k = i / h;
-                    c = px.L + k; r = py.L + (i - k * h);
-                    word = mbox_col_word(r, c);
-                } else {
-                    const int ww = px.R - px.D, j = i - n_col;
-                    const int k = j / ww;
-                    r = py.L + k; c = px.D + (j - k * ww);
-                    word = mbox_row_word(r, c);
+        int bad = 0;
+        if (warp < CV_NCW) {
+            // ---- compute warps: the windows of step g ---------------------------------------------------
+            const AxisEntry ey = sm.tab[g % CV_TR][0], ex = sm.tab[g % CV_TR][1];
+            if (ey.nw > 0 && ex.nw > 0) {
+                const CFamily fam = sm.fams[f];
+                float *qplane = p.q + (size_t)f * plane + frame_off_q;
+                const float *qst = sm.qs[g % CV_NST];
+                const bool first = g < p.F;
+                switch (fam.side) {
+                    case 1: project_tile<1, 8>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
+                    case 2: project_tile<2, 4>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
+                    case 3: project_tile<3, 3>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
+                    case 4: project_tile<4, 2>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
+                    case 5: project_tile<5, 2>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
+                    case 6: project_tile<6, 1>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
+                    case 7: project_tile<7, 1>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
+                    case 8: project_tile<8, 1>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
+                    default:
+                        if (fam.G <= 16) project_tile_big<16>(sm, qst, qplane, ey, ex, fam.side, fam.c, fam.sqrt_c, p.Wq, first, warp, lane);
+                        else project_tile_big<32>(sm, qst, qplane, ey, ex, fam.side, fam.c, fam.sqrt_c, p.Wq, first, warp, lane);
                 }
-                const int which = (c < px.D ? 1 : 0) | (r < py.D ? 2 : 0);    // 1 left, 2 up, 3 up-left
-                if ((int)sm.nbr_prog[which] + CV_D < g)              // ring slot still unread by the receiver?
-                    poll_prog(p.prog + nbr_cta(which), (unsigned)(g - CV_D), p.status);
-                const unsigned long long wv = ((unsigned long long)(unsigned)g << 32) | __float_as_uint(sm.xs[tidx(r, c)]);
-                st_u64_gpu(p.mbox + ((size_t)nbr_cta(which) * CV_D + (g % CV_D)) * CV_MBW + word, wv);
             }
-        }
-
-        // ---- (a) prefetch q of step g + CV_PF and the table entry of step g + CV_LA ---------------------
-        {
+        } else if (warp == CV_NCW) {
+            // ---- loader warp: q of step g + CV_PF and the table entry of step g + CV_LA + 1 ---------------
             const int gp = g + CV_PF;
             if (gp < total && gp >= p.F) {                           // the first sweep reads no q (q = 0)
                 const AxisEntry qy = sm.tab[gp % CV_TR][0], qx = sm.tab[gp % CV_TR][1];
-                const CFamily qf = sm.fams[fp];
                 if (qy.nw > 0 && qx.nw > 0) {
-                    const int rows = qy.nw * qf.side;
-                    const int c0 = qx.w0 & ~3, c1 = (qx.w0 + qx.nw * qf.side + 3) & ~3;
-                    const int nch = (c1 - c0) >> 2;
-                    const float *src = p.q + (size_t)fp * plane + frame_off_q;
-                    const unsigned dst = (unsigned)__cvta_generic_to_shared(sm.qs[gp % CV_NST]);
-                    for (int i = tid; i < rows * nch; i += CV_NT) {
-                        const int rr = i / nch, ch = i - rr * nch;
-                        const int r = qy.w0 + rr, c = c0 + 4 * ch;
-                        if (c < p.Wq)
-                            cp_async16(dst + 4u * (unsigned)tidx(r, c), src + (size_t)r * p.Wq + c);
+                    const int s = sm.fams[fp].side;
+                    const int rows = qy.nw * s;
+                    const int c0 = qx.w0 & ~3, c1 = (qx.w0 + qx.nw * s + 3) & ~3;
+                    const int half = lane >> 4, ch = lane & 15;      // 16 chunks of 4 columns cover a row
+                    const int c = c0 + 4 * ch;
+                    if (c < c1 && c < p.Wq) {
+                        const float *src = p.q + (size_t)fp * plane + frame_off_q + (size_t)(qy.w0 + half) * p.Wq + c;
+                        unsigned dst = (unsigned)__cvta_generic_to_shared(sm.qs[gp % CV_NST]) + 4u * (unsigned)(half * CV_PW + 4 * ch);
+                        for (int rr = half; rr < rows; rr += 2) {
+                            cp_async16(dst, src);
+                            dst += 2 * CV_PW * 4;
+                            src += 2 * (size_t)p.Wq;
+                        }
                     }
                 }
             }
             const int gt = g + CV_LA + 1;
-            if (gt < total && tid < 2) {
-                const AxisEntry *src = tid ? p.tabx + (size_t)gt * p.NC + cj : p.taby + (size_t)gt * p.NR + ci;
-                cp_async16((unsigned)__cvta_generic_to_shared(&sm.tab[gt % CV_TR][tid]), src);
+            if (gt < total && lane < 2) {
+                const AxisEntry *src = lane ? p.tabx + (size_t)gt * p.NC + cj : p.taby + (size_t)gt * p.NR + ci;
+                cp_async16((unsigned)__cvta_generic_to_shared(&sm.tab[gt % CV_TR][lane]), src);
             }
             cp_async_commit();
-        }
-
-        // ---- (c) the windows of step g ----------------------------------------------------------------
-        if (ey.nw > 0 && ex.nw > 0) {
-            float *qplane = p.q + (size_t)f * plane + frame_off_q;
-            const float *qst = sm.qs[g % CV_NST];
-            const bool first = g < p.F;
-            switch (fam.G) {
-                case 1: project_tile<1>(sm, qst, qplane, ey, ex, fam, p.Wq, first); break;
-                case 2: project_tile<2>(sm, qst, qplane, ey, ex, fam, p.Wq, first); break;
-                case 4: project_tile<4>(sm, qst, qplane, ey, ex, fam, p.Wq, first); break;
-                case 8: project_tile<8>(sm, qst, qplane, ey, ex, fam, p.Wq, first); break;
-                case 16: project_tile<16>(sm, qst, qplane, ey, ex, fam, p.Wq, first); break;
-                default: project_tile<32>(sm, qst, qplane, ey, ex, fam, p.Wq, first); break;
+            cp_async_wait<CV_PF - 1>();                              // q of step g+1 has landed
+        } else if (warp == CV_NCW + 1) {
+            // ---- sender warp: departures of step g-1 -> the neighbours' mailboxes, tagged g --------------
+            if (g > 0) {
+                if (lane >= 1 && lane <= 3) {                        // the ring slot must have been read
+                    // the neighbour's counter is re-read only when the ring is half used, and the value is
+                    // picked up a few steps later: the load must never sit on this warp's critical path
+                    if (prog_iter >= 0 && g >= prog_iter + 3) { prog_seen = max(prog_seen, prog_pend); prog_iter = -1; }
+                    if ((int)prog_seen + CV_D < g) {
+                        prog_seen = poll_prog(p.prog + (size_t)nbr_cta(lane) * CV_PROG_STRIDE, (unsigned)(g - CV_D), p.status);
+                        prog_iter = -1;
+                    } else if (prog_iter < 0 && (int)prog_seen + CV_D / 2 < g) {
+                        prog_pend = ld_u32_gpu(p.prog + (size_t)nbr_cta(lane) * CV_PROG_STRIDE);
+                        prog_iter = g;
+                    }
+                }
+                __syncwarp();
+                if (p.trace && lane == 0) {
+                    unsigned long long t;
+                    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+                    p.trace[((size_t)cta * total + g) * 8 + 6] = t;
+                }
+                const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
+                const size_t slot = (size_t)(g % CV_D) * CV_MBW;
+                const unsigned long long tag = (unsigned long long)(unsigned)g << 32;
+                for (int c = px.L; c < px.D; ++c)                    // column strip: columns [L, D), all rows
+                    for (int r = py.L + lane; r < py.R; r += 32) {
+                        const int which = 1 | (r < py.D ? 2 : 0);
+                        st_u64_gpu(p.mbox + (size_t)nbr_cta(which) * CV_D * CV_MBW + slot + mbox_col_word(r, c),
+                                   tag | __float_as_uint(sm.xs[tidx(r, c)]));
+                    }
+                for (int r = py.L; r < py.D; ++r)                    // row strip: rows [L, D), columns [D, R)
+                    for (int c = px.D + lane; c < px.R; c += 32)
+                        st_u64_gpu(p.mbox + (size_t)nbr_cta(2) * CV_D * CV_MBW + slot + mbox_row_word(r, c),
+                                   tag | __float_as_uint(sm.xs[tidx(r, c)]));
             }
-        }
-
-        // ---- (d) arrivals of step g+1 into the tile; start loading the arrivals of step g+2 ------------
-        if (g + 1 < total) {
-            const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
-            const int n_col = (ny.R - ny.L) * (nx.R - nx.A);
-            const int n_arr = n_col + (ny.R - ny.A) * (nx.A - nx.L);
-            const unsigned long long *box = my_box + (size_t)((g + 1) % CV_D) * CV_MBW;
-            for (int i = hi; i < n_arr; i += CV_NT) {
-                int r, c, word;
-                arrival(ny, nx, i, n_col, r, c, word);
-                unsigned long long wv = (i == hi) ? pend : 0ull;
-                if ((unsigned)(wv >> 32) != (unsigned)(g + 1)) wv = poll_tag(box + word, (unsigned)(g + 1), p.status);
-                sm.xs[tidx(r, c)] = __uint_as_float((unsigned)wv);
-            }
-            pend = 0;
-            if (g + 2 < total) {
-                const AxisEntry my = sm.tab[(g + 2) % CV_TR][0], mx = sm.tab[(g + 2) % CV_TR][1];
-                const int m_col = (my.R - my.L) * (mx.R - mx.A);
-                const int m_arr = m_col + (my.R - my.A) * (mx.A - mx.L);
-                if (hi < m_arr) {
-                    int r, c, word;
-                    arrival(my, mx, hi, m_col, r, c, word);
-                    pend = ld_u64_gpu(my_box + (size_t)((g + 2) % CV_D) * CV_MBW + word);
+        } else {
+            // ---- receiver warp: arrivals of step g+1 into the tile; preload the first line of step g+2 ----
+            if (g + 1 < total) {
+                const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
+                const unsigned long long *box = my_box + (size_t)((g + 1) % CV_D) * CV_MBW;
+                const unsigned tag = (unsigned)(g + 1);
+                bool first_line = true;
+                for (int c = nx.A; c < nx.R; ++c) {                  // column strip: columns [A, R), all rows
+                    for (int r = ny.L + lane, t = 0; r < ny.R; r += 32, ++t) {
+                        unsigned long long wv = (first_line && t < 2) ? (t ? pend1 : pend0) : 0ull;
+                        if ((unsigned)(wv >> 32) != tag) wv = poll_tag(box + mbox_col_word(r, c), tag, p.status);
+                        sm.xs[tidx(r, c)] = __uint_as_float((unsigned)wv);
+                    }
+                    first_line = false;
+                }
+                for (int r = ny.A; r < ny.R; ++r) {                  // row strip: rows [A, R), columns [L, A)
+                    for (int c = nx.L + lane, t = 0; c < nx.A; c += 32, ++t) {
+                        unsigned long long wv = (first_line && t < 2) ? (t ? pend1 : pend0) : 0ull;
+                        if ((unsigned)(wv >> 32) != tag) wv = poll_tag(box + mbox_row_word(r, c), tag, p.status);
+                        sm.xs[tidx(r, c)] = __uint_as_float((unsigned)wv);
+                    }
+                    first_line = false;
+                }
+                __syncwarp();
+                if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // mailbox of step g+1 has been read
+                pend0 = pend1 = 0;
+                if (g + 2 < total) {
+                    const AxisEntry my = sm.tab[(g + 2) % CV_TR][0], mx = sm.tab[(g + 2) % CV_TR][1];
+                    const unsigned long long *box2 = my_box + (size_t)((g + 2) % CV_D) * CV_MBW;
+                    if (mx.A < mx.R) {                               // first line = first arriving column
+                        const int r = my.L + lane;
+                        if (r < my.R) pend0 = ld_u64_gpu(box2 + mbox_col_word(r, mx.A));
+                        if (r + 32 < my.R) pend1 = ld_u64_gpu(box2 + mbox_col_word(r + 32, mx.A));
+                    } else if (my.A < my.R) {                        // ... or the first arriving row
+                        const int c = mx.L + lane;
+                        if (c < mx.A) pend0 = ld_u64_gpu(box2 + mbox_row_word(my.A, c));
+                        if (c + 32 < mx.A) pend1 = ld_u64_gpu(box2 + mbox_row_word(my.A, c + 32));
+                    }
                 }
             }
+            if (lane == 0) { bad = status_pend; status_pend = *(volatile int *)p.status; }
         }
 
-        // ---- bookkeeping loads, consumed one iteration later ------------------------------------------
-        int bad = 0;
-        if (tid == 0) { bad = status_pend; status_pend = *(volatile int *)p.status; }
-        if (tid >= 1 && tid <= 3) {
-            sm.nbr_prog[tid] = prog_pend;
-            prog_pend = ld_u32_gpu(p.prog + nbr_cta(tid));
+        // ---- one barrier per step ----------------------------------------------------------------------
+        if (p.trace && lane == 0 && (warp == 0 || warp >= CV_NCW - 1)) {      // debug: when each role finished
+            unsigned long long t;
+            asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+            p.trace[((size_t)cta * total + g) * 8 + 1 + (warp == 0 ? 0 : warp - (CV_NCW - 2))] = t;
         }
-
-        // ---- (e) one barrier per step; q of step g+1 has landed -----------------------------------------
-        cp_async_wait<CV_PF - 1>();
         if (__syncthreads_or(bad)) return;
-        if (tid == 0) st_u32_gpu(p.prog + cta, (unsigned)(g + 1));   // mailbox of step g+1 has been read
-
+        if (p.trace && tid == 0) {
+            unsigned long long t;
+            asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+            p.trace[((size_t)cta * total + g) * 8] = t;
+        }
         if (++f == p.F) f = 0;
         if (++fp == p.F) fp = 0;
     }
@@ -451,7 +526,7 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
     const bool good =
         cudaMalloc(&pl->d_fams, cf.size() * sizeof(CFamily)) == cudaSuccess &&
         cudaMalloc(&pl->d_mbox, pl->mbox_bytes) == cudaSuccess &&
-        cudaMalloc(&pl->d_prog, n_cta * sizeof(unsigned)) == cudaSuccess &&
+        cudaMalloc(&pl->d_prog, n_cta * CV_PROG_STRIDE * sizeof(unsigned)) == cudaSuccess &&
         cudaMalloc(&pl->d_status, sizeof(int)) == cudaSuccess &&
         cudaMemcpy(pl->d_fams, cf.data(), cf.size() * sizeof(CFamily), cudaMemcpyHostToDevice) == cudaSuccess &&
         cudaMemset(pl->d_status, 0, sizeof(int)) == cudaSuccess;
@@ -504,17 +579,31 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
     p.F = pl->F; p.total = pl->F * n_sweeps; p.H = pl->H; p.W = pl->W; p.Wq = pl->Wq; p.B_total = pl->B;
     p.NR = pl->NR; p.NC = pl->NC;
     const int tiles = pl->NR * pl->NC;
+    const char *trace_path = getenv("SMRE_CV_TRACE");        // debug only: synchronises and writes a file
+    if (trace_path && cudaMalloc(&p.trace, (size_t)tiles * p.total * 64) != cudaSuccess) p.trace = nullptr;
     for (int f0 = 0; f0 < pl->B; f0 += pl->frames_per_launch) {
         p.frame0 = f0;
         const int nb = std::min(pl->frames_per_launch, pl->B - f0);
         // tags and progress counters restart in every launch
         if ((e = cudaMemsetAsync(pl->d_mbox, 0, (size_t)nb * tiles * CV_D * CV_MBW * 8, st)) != cudaSuccess) return e;
-        if ((e = cudaMemsetAsync(pl->d_prog, 0, (size_t)nb * tiles * sizeof(unsigned), st)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(pl->d_prog, 0, (size_t)nb * tiles * CV_PROG_STRIDE * sizeof(unsigned), st)) != cudaSuccess) return e;
         void *args[] = {&p};
         e = cudaLaunchCooperativeKernel((const void *)conveyor_kernel, dim3((unsigned)(nb * tiles)),
                                         dim3(CV_NT), args, sizeof(Smem), st);
         if (e != cudaSuccess) return e;
         if (launches) ++*launches;
+    }
+    if (p.trace) {
+        std::vector<unsigned long long> t((size_t)tiles * p.total * 8);
+        cudaStreamSynchronize(st);
+        cudaMemcpy(t.data(), p.trace, t.size() * 8, cudaMemcpyDeviceToHost);
+        cudaFree(p.trace);
+        if (FILE *fh = fopen(trace_path, "wb")) {
+            const int hdr[4] = {pl->NR, pl->NC, p.total, pl->F};
+            fwrite(hdr, sizeof hdr, 1, fh);
+            fwrite(t.data(), 8, t.size(), fh);
+            fclose(fh);
+        }
     }
     return cudaSuccess;
 }

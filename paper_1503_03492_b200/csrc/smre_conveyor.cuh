@@ -9,7 +9,8 @@
 
 namespace smre {
 
-constexpr int CV_NT = 512;              // threads per CTA
+constexpr int CV_NCW = 16;              // compute warps per CTA
+constexpr int CV_NT = (CV_NCW + 3) * 32;    // + one loader, one sender, one receiver warp
 constexpr int CV_PW = 64;               // edge of the torus-addressed x tile in shared memory
 constexpr int CV_SD = 16;               // strip depth: a boundary moves < CV_SD pixels per step
 constexpr int CV_D = 16;                // mailbox ring depth (steps)
@@ -18,6 +19,7 @@ constexpr int CV_NST = CV_PF + 1;       // q stages in shared memory
 constexpr int CV_TR = 16;               // table ring entries in shared memory
 constexpr int CV_LA = 2 * CV_PF + 1;    // table look-ahead (steps)
 constexpr int CV_MBW = 2 * CV_SD * CV_PW;   // 8-byte words per mailbox slot
+constexpr int CV_PROG_STRIDE = 64;       // progress counters 256 bytes apart: no line is shared by two CTAs
 constexpr int CV_MAX_F = 1024;          // families kept in shared memory
 
 // One axis of one tile slot at one step (16 bytes).  All positions are clipped to [0, N].
