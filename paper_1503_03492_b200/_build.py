@@ -27,6 +27,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
+        if os.environ.get("SMRE_CV_TRACE_BUILD"):
+            cmd.insert(1, "-DSMRE_CV_TRACE_BUILD")
         if os.environ.get("SMRE_DEBUG"):
             cmd.insert(1, "-DSMRE_DEBUG")
         else:

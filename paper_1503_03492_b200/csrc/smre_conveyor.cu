@@ -23,6 +23,7 @@
 // scheduler and the graph scheduler return identical bits.
 #include "smre_conveyor.cuh"
 
+#include <cuda.h>          // CUtensorMap (types only; the encoder is fetched with cudaGetDriverEntryPoint)
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -30,9 +31,12 @@
 
 namespace smre {
 
-struct CFamily {
-    int side, G;                  // window edge; lanes per window (power of two >= side)
+struct CFamily {                  // 32 bytes
+    int side, lgG;                // window edge; log2 of the lanes per window (power of two >= side)
+    int run_left;                 // families from this one to the end of its run of equal edges (within a sweep)
+    int pad0;
     float c, sqrt_c;
+    int pad1[2];
 };
 
 struct CParams {
@@ -49,6 +53,8 @@ struct CParams {
     int F, total;
     int H, W, Wq, B_total, frame0;   // Wq: row pitch of the q planes (W rounded up to 4)
     int NR, NC;
+    int qp;                       // row pitch (floats) of a q stage in shared memory = columns of a TMA box
+    CUtensorMap qmap[8];          // q as a 2-D tensor [F*B*H rows][Wq]; box = qp columns x 8*(k+1) rows
 };
 
 // ---- small PTX helpers ---------------------------------------------------------------------------
@@ -74,6 +80,25 @@ __device__ __forceinline__ void cp_async16(unsigned smem_addr, const void *gptr)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// ---- mbarrier + TMA (the q boxes) ----------------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(unsigned long long *bar, unsigned parity) {
+    unsigned ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void tma_load_2d(void *smem_dst, const CUtensorMap *map, int c0, int c1, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(map), "r"(c0), "r"(c1),
+                   "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
 
 // Spin until the mailbox word carries `tag`.  A poll that outlives ~1 s (or sees another CTA's failure)
 // raises *status and gives up, so a protocol bug cannot hang the GPU.
@@ -114,123 +139,282 @@ static_assert(CV_PW == 64, "tidx assumes a 64 x 64 torus");
 __device__ __forceinline__ int mbox_col_word(int r, int c) { return ((c & (CV_SD - 1)) << 6) | (r & 63); }
 __device__ __forceinline__ int mbox_row_word(int r, int c) { return CV_SD * 64 + (((r & (CV_SD - 1)) << 6) | (c & 63)); }
 
+// Per-step descriptor (32 bytes = two 16-byte broadcast loads), written one step ahead by the control
+// warp so that the compute warps do almost no index arithmetic of their own.
+struct StepDesc {
+    // v0
+    int geom;                     // changes whenever (side, window counts) change: lanes re-derive their item then
+    int n_items;                  // lanes of work (blocks of window rows * windows per row * G); 0: nothing
+    int w0yx;                     // origin of the first window: row | column << 16
+    unsigned qbase;               // float offset in Smem::qs of (first window row, first window column) of this step's box;
+                                  // bit 31: first sweep (q is zero and is not read)
+    // v1
+    unsigned goff_lo, goff_hi;    // element offset in q of (family plane, frame, first window row, first window column)
+    int f;                        // family index of this step
+    int run_left;                 // steps left in this run of equal window edges, this one included
+};
+static_assert(sizeof(StepDesc) == 32, "StepDesc must be 32 bytes");
+
+struct GeomDesc { int nwx, nwy, n_items, pad; };   // read by the lanes only when StepDesc::geom changes
+
 struct Smem {
     float xs[CV_PW * CV_PW];                 // the x tile, torus addressed by image (row, column)
-    float qs[CV_NST][CV_PW * CV_PW];         // q stages: [(row - first window row) * 64 + (column - c0)]
+    float qs[CV_NST * CV_PW * CV_PW];        // q stages, filled by TMA: [(row - first window row) * qp + (column - c0)], c0 = first window column rounded down to 4
     AxisEntry tab[CV_TR][2];                 // [step % CV_TR][0 = y, 1 = x]
+    StepDesc desc[2];                        // [step & 1]
+    GeomDesc geo[2];                         // [geom & 1]
+    unsigned long long qbar[CV_NST];         // mbarriers: the TMA box of a stage has landed
     CFamily fams[CV_MAX_F];
+    int abort;                               // set by the receiver warp when the failure flag is up
 };
 
-// The windows of one step inside this CTA's tile, for a compile-time window edge S.
-// G = lanes per window (power of two >= S): lane j of a window owns column j.  A lane handles KR
-// vertically stacked windows (S * KR rows of its column) so that the per-item index arithmetic is
-// paid once per ~8 pixels whatever the window size.  Summation order per window = family_pass_kernel's:
-// rows top to bottom inside the lane (fma), then an xor-shuffle tree over the G lanes.
-template <int S, int KR>
-__device__ __forceinline__ void project_tile(Smem &sm, const float *qst, float *__restrict__ qplane,
-                                             const AxisEntry &ey, const AxisEntry &ex, float c, float sqrt_c,
-                                             int Wq, bool first_sweep, int cw, int lane)
+// One barrier per step.  Every 8th step all warps also look at Smem::abort (set only at steps = 3 mod 8,
+// so that every warp reads the same value) and leave together if a hand-off has timed out somewhere.
+#define CV_STEP_BARRIER()                                                         \
+    do {                                                                          \
+        __syncthreads();                                                          \
+        if ((g & 7) == 7 && *(volatile int *)&sm.abort) return;                   \
+    } while (0)
+
+#ifdef SMRE_CV_TRACE_BUILD
+#define CV_STAMP(slot)                                                            \
+    do {                                                                          \
+        if (p.trace) {                                                            \
+            unsigned long long t_;                                                \
+            asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_));                 \
+            p.trace[((size_t)cta * total + g) * 8 + (slot)] = t_;                 \
+        }                                                                         \
+    } while (0)
+#else
+#define CV_STAMP(slot) ((void)0)
+#endif
+
+// One item = one lane's column of KR vertically stacked windows of edge S (rows masked onto the torus).
+// Summation order per window = family_pass_kernel's: rows top to bottom inside the lane (fma), then an
+// xor-shuffle tree over the G lanes of the window.
+template <int S, int KR, int G, int WQ>
+__device__ __forceinline__ void project_item(float *xs, const float *qs0, float *__restrict__ qg, int xi0,
+                                             int nwin, float c, float sqrt_c, int Wq_rt, int qp_rt, bool first_sweep)
 {
-    constexpr int G = S <= 1 ? 1 : S <= 2 ? 2 : S <= 4 ? 4 : 8;
     constexpr int R = S * KR;
-    const int nwy = ey.nw, nwx = ex.nw;
-    const int nby = (nwy + KR - 1) / KR;                 // blocks of KR window rows
-    const int n_items = nby * nwx * G;
-    const int c0 = ex.w0 & ~3;
-    for (int base = cw * 32; base < n_items; base += CV_NCW * 32) {
+    const int Wq = WQ ? WQ : Wq_rt;
+    const int qp = WQ ? CV_PW : qp_rt;                     // q stage pitch: 64 whenever the pitch of q is templated
+    float v[R], part[KR];
+#pragma unroll
+    for (int k = 0; k < KR; ++k) {
+        part[k] = 0.0f;
+#pragma unroll
+        for (int r = 0; r < S; ++r) {
+            const int rr = k * S + r;
+            v[rr] = 0.0f;
+            if (k < nwin) {
+                const float xv = xs[(xi0 + rr * CV_PW) & (CV_PW * CV_PW - 1)];
+                v[rr] = first_sweep ? xv : xv + qs0[rr * qp];
+            }
+            part[k] = fmaf(v[rr], v[rr], part[k]);
+        }
+    }
+#pragma unroll
+    for (int m = G / 2; m > 0; m >>= 1)
+#pragma unroll
+        for (int k = 0; k < KR; ++k) part[k] += __shfl_xor_sync(0xffffffffu, part[k], m);
+#pragma unroll
+    for (int k = 0; k < KR; ++k) {
+        const float alpha = ball_scale(part[k], c, sqrt_c);
+#pragma unroll
+        for (int r = 0; r < S; ++r) {
+            const int rr = k * S + r;
+            if (k < nwin) {
+                const float xn = alpha * v[rr];
+                xs[(xi0 + rr * CV_PW) & (CV_PW * CV_PW - 1)] = xn;
+                __stcs(qg + rr * Wq, v[rr] - xn);
+            }
+        }
+    }
+}
+
+// Window edges above 8 (G = 16 or 32 lanes per window, run-time edge s, one window per lane group) and any
+// item beyond the first CV_NCW * 32 of a step: the generic, un-cached path.
+template <int G>
+__device__ __forceinline__ void project_generic(Smem &sm, const GeomDesc &ge, int s, int kr, int w0y, int w0x,
+                                                const float *qst, float *__restrict__ qplane, float c,
+                                                float sqrt_c, int Wq, int qp, bool first_sweep, int base0, int cw, int lane)
+{
+    for (int base = base0 + cw * 32; base < ge.n_items; base += CV_NCW * 32) {
         const int item = base + lane;
         const int grp = item / G, j = item % G;
-        const int by = (int)(((unsigned)grp * ex.magic) >> 20), wix = grp - by * nwx;
-        const bool on = item < n_items && j < S;
-        const int nwin = on ? min(KR, nwy - by * KR) : 0;    // valid windows of this block
-        const int rr0 = by * R;
-        const int r0 = ey.w0 + rr0, cc = ex.w0 + wix * S + j;
-        const int xi0 = tidx(r0, cc);
-        const float *qs0 = qst + rr0 * CV_PW + (cc - c0);
-        float *qg = qplane + (size_t)r0 * Wq + cc;
-        float v[R], part[KR];
+        const int by = grp / ge.nwx, wix = grp - by * ge.nwx;
+        const bool on = item < ge.n_items && j < s;
+#pragma unroll 1
+        for (int k = 0; k < kr; ++k) {                       // stacked windows, one at a time
+            const bool act = on && by * kr + k < ge.nwy;
+            const int rr0 = (by * kr + k) * s;
+            const int r0 = w0y + rr0, cc = w0x + wix * s + j;
+            const int xi0 = tidx(r0, cc);
+            const float *qs0 = qst + rr0 * qp + (wix * s + j);
+            float *qg = qplane + (rr0 * Wq + wix * s + j);
+            float v[G];
+            float part = 0.0f;
 #pragma unroll
-        for (int k = 0; k < KR; ++k) {
-            part[k] = 0.0f;
-#pragma unroll
-            for (int r = 0; r < S; ++r) {
-                const int rr = k * S + r;
-                v[rr] = 0.0f;
-                if (k < nwin) {
-                    const float xv = sm.xs[(xi0 + rr * CV_PW) & (CV_PW * CV_PW - 1)];
-                    v[rr] = first_sweep ? xv : xv + qs0[rr * CV_PW];
+            for (int r = 0; r < G; ++r) {
+                v[r] = 0.0f;
+                if (r < s && act) {
+                    const float xv = sm.xs[(xi0 + r * CV_PW) & (CV_PW * CV_PW - 1)];
+                    v[r] = first_sweep ? xv : xv + qs0[r * qp];
                 }
-                part[k] = fmaf(v[rr], v[rr], part[k]);
+                part = fmaf(v[r], v[r], part);
             }
-        }
 #pragma unroll
-        for (int m = G / 2; m > 0; m >>= 1)
+            for (int m = G / 2; m > 0; m >>= 1) part += __shfl_xor_sync(0xffffffffu, part, m);
+            const float alpha = ball_scale(part, c, sqrt_c);
 #pragma unroll
-            for (int k = 0; k < KR; ++k) part[k] += __shfl_xor_sync(0xffffffffu, part[k], m);
-#pragma unroll
-        for (int k = 0; k < KR; ++k) {
-            const float alpha = ball_scale(part[k], c, sqrt_c);
-#pragma unroll
-            for (int r = 0; r < S; ++r) {
-                const int rr = k * S + r;
-                if (k < nwin) {
-                    const float xn = alpha * v[rr];
-                    sm.xs[(xi0 + rr * CV_PW) & (CV_PW * CV_PW - 1)] = xn;
-                    __stcs(qg + (size_t)rr * Wq, v[rr] - xn);
+            for (int r = 0; r < G; ++r) {
+                if (r < s && act) {
+                    const float xn = alpha * v[r];
+                    sm.xs[(xi0 + r * CV_PW) & (CV_PW * CV_PW - 1)] = xn;
+                    __stcs(qg + r * Wq, v[r] - xn);
                 }
             }
         }
     }
 }
 
-// Window edges above 8: G = 16 or 32 lanes per window, run-time edge s, one window per lane group.
-template <int G>
-__device__ __forceinline__ void project_tile_big(Smem &sm, const float *qst, float *__restrict__ qplane,
-                                                 const AxisEntry &ey, const AxisEntry &ex, int s, float c,
-                                                 float sqrt_c, int Wq, bool first_sweep, int cw, int lane)
+// State of one compute lane that survives from step to step.
+struct LaneCache {
+    int geom;                     // geometry id the fields below were derived for
+    int nwin;                     // valid stacked windows of this lane's first item (0: lane idle)
+    int busy;                     // warp-uniform: this warp has an item at all
+    int rr0, colofs;              // row / column of the item relative to the first window's origin
+    int lq, lg;                   // rr0 * qp + colofs,  rr0 * Wq + colofs
+};
+
+// A run of steps [g, g_end) that share the window edge S, for one compute warp.
+template <int S, int KR, int WQ>
+__device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache &lc, int &g, int g_end, float c,
+                                          float sqrt_c, int warp, int lane, int cta, int total)
 {
-    const int nwx = ex.nw;
-    const int n_items = ey.nw * nwx * G;
-    const int c0 = ex.w0 & ~3;
-    for (int base = cw * 32; base < n_items; base += CV_NCW * 32) {
-        const int item = base + lane;
-        const int win = item / G, j = item % G;
-        const int wiy = (int)(((unsigned)win * ex.magic) >> 20), wix = win - wiy * nwx;
-        const bool on = item < n_items && j < s;
-        const int rr0 = wiy * s;
-        const int r0 = ey.w0 + rr0, cc = ex.w0 + wix * s + j;
-        const int xi0 = tidx(r0, cc);
-        const float *qs0 = qst + rr0 * CV_PW + (cc - c0);
-        float *qg = qplane + (size_t)r0 * Wq + cc;
-        float v[G];
-        float part = 0.0f;
-#pragma unroll
-        for (int r = 0; r < G; ++r) {
-            v[r] = 0.0f;
-            if (r < s && on) {
-                const float xv = sm.xs[(xi0 + r * CV_PW) & (CV_PW * CV_PW - 1)];
-                v[r] = first_sweep ? xv : xv + qs0[r * CV_PW];
-            }
-            part = fmaf(v[r], v[r], part);
+    constexpr int G = S <= 1 ? 1 : S <= 2 ? 2 : S <= 4 ? 4 : 8;
+    constexpr int LG = S <= 1 ? 0 : S <= 2 ? 1 : S <= 4 ? 2 : 3;
+    const int Wq = WQ ? WQ : p.Wq;
+    const int qp = WQ ? CV_PW : p.qp;
+    for (; g < g_end; ++g) {
+        const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g & 1].geom);
+        if (warp == 0 && lane == 0) CV_STAMP(6);
+        if ((int)v0.x != lc.geom) {                            // rare: the tile's window counts changed
+            const GeomDesc ge = sm.geo[v0.x & 1];
+            const int n_items = (int)v0.y;
+            lc.geom = (int)v0.x;
+            const int item = warp * 32 + lane;
+            const int grp = item >> LG, j = item & (G - 1);
+            const int by = ge.nwx > 0 ? grp / ge.nwx : 0, wix = grp - by * ge.nwx;
+            const bool on = item < n_items && j < S;
+            lc.nwin = on ? min(KR, ge.nwy - by * KR) : 0;
+            lc.busy = warp * 32 < n_items;
+            lc.rr0 = by * KR * S;
+            lc.colofs = wix * S + j;
+            lc.lq = lc.rr0 * qp + lc.colofs;
+            lc.lg = lc.rr0 * Wq + lc.colofs;
         }
-#pragma unroll
-        for (int m = G / 2; m > 0; m >>= 1) part += __shfl_xor_sync(0xffffffffu, part, m);
-        const float alpha = ball_scale(part, c, sqrt_c);
-#pragma unroll
-        for (int r = 0; r < G; ++r) {
-            if (r < s && on) {
-                const float xn = alpha * v[r];
-                sm.xs[(xi0 + r * CV_PW) & (CV_PW * CV_PW - 1)] = xn;
-                __stcs(qg + (size_t)r * Wq, v[r] - xn);
-            }
+        if (lc.busy) {
+            const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g & 1].goff_lo);
+            const int r0 = (int)(v0.z & 0xffffu) + lc.rr0, cc = (int)(v0.z >> 16) + lc.colofs;
+            const float *qs0 = sm.qs + (v0.w & 0x7fffffffu) + lc.lq;
+            float *qg = p.q + (((unsigned long long)v1.y << 32) | v1.x) + lc.lg;
+            project_item<S, KR, G, WQ>(sm.xs, qs0, qg, tidx(r0, cc), lc.nwin, c, sqrt_c, p.Wq, p.qp, (v0.w >> 31) != 0);
+            if ((int)v0.y > CV_NCW * 32)
+                project_generic<G>(sm, sm.geo[v0.x & 1], S, KR, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
+                                   sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
+                                   c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, CV_NCW * 32, warp, lane);
         }
+        if (warp == 0 && lane == 0) CV_STAMP(1);
+        if (warp == 8 && lane == 0) CV_STAMP(2);
+        CV_STEP_BARRIER();
+        if (warp == 0 && lane == 0) CV_STAMP(0);
     }
 }
 
+// Window edges above 8: same loop, generic arithmetic only.
+template <int G, int WQ>
+__device__ __forceinline__ void run_steps_big(Smem &sm, const CParams &p, int s, int &g, int g_end, float c,
+                                              float sqrt_c, int warp, int lane, int cta, int total)
+{
+    const int Wq = WQ ? WQ : p.Wq;
+    const int qp = WQ ? CV_PW : p.qp;
+    for (; g < g_end; ++g) {
+        const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g & 1].geom);
+        const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g & 1].goff_lo);
+        if ((int)v0.y > 0)
+            project_generic<G>(sm, sm.geo[v0.x & 1], s, 1, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
+                               sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
+                               c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, 0, warp, lane);
+        CV_STEP_BARRIER();
+    }
+}
+
+// Control lane: the descriptor of step g (family f, q stage st = g % CV_NST).
+struct ControlState {
+    int geom, key;                     // geometry id and what it stands for
+    unsigned long long plane_f;        // f * plane + frame offset (elements)
+    int row_fp;                        // tensor row of (family fp, frame, row 0): (fp * B_total + frame) * H
+    unsigned phase;                    // bit s: parity the next wait on q stage s has to use
+};
+__device__ __forceinline__ void make_desc(Smem &sm, const CParams &p, ControlState &cs, int g, int f, int st,
+                                          int total)
+{
+    const AxisEntry ey = sm.tab[g % CV_TR][0], ex = sm.tab[g % CV_TR][1];
+    const CFamily fam = sm.fams[f];
+    StepDesc d;
+    const int n_items = (ey.nw > 0 && ex.nw > 0) ? (ey.e0 * ex.nw) << fam.lgG : 0;
+    const int key = (fam.side << 16) | (ey.nw << 8) | ex.nw;
+    if (key != cs.key) {
+        cs.key = key; ++cs.geom;
+        GeomDesc ge; ge.nwx = ex.nw; ge.nwy = ey.nw; ge.n_items = n_items; ge.pad = 0;
+        sm.geo[cs.geom & 1] = ge;
+    }
+    d.geom = cs.geom; d.n_items = n_items;
+    d.w0yx = ey.w0 | (ex.w0 << 16);
+    d.qbase = (unsigned)(st * (CV_PW * CV_PW) + (ex.w0 - ex.e0)) | (g < p.F ? 0x80000000u : 0u);
+    const unsigned long long goff = cs.plane_f + (unsigned)(ey.w0 * p.Wq + ex.w0);
+    d.goff_lo = (unsigned)goff; d.goff_hi = (unsigned)(goff >> 32);
+    d.f = f; d.run_left = min(fam.run_left, total - g);
+    sm.desc[g & 1] = d;
+}
+
+// Does step g read q through a TMA box (issued CV_PF steps earlier, awaited just before the step)?
+__device__ __forceinline__ bool step_loads_q(const Smem &sm, const CParams &p, int g, int total)
+{
+    if (g < p.F || g >= total) return false;                         // the first sweep reads no q (q = 0)
+    return sm.tab[g % CV_TR][0].nw > 0 && sm.tab[g % CV_TR][1].nw > 0;
+}
+
+// Arrival chunk k of the step described by (Y, X): 32 consecutive positions of one line.  Lines: the
+// columns [X.A, X.R) of the column strip (all tile rows), then the rows [Y.A, Y.R) of the row strip
+// (columns [X.L, X.A)); two chunks per line (tiles are at most 64 wide / tall).
+__device__ __forceinline__ bool arrival_chunk(const AxisEntry &Y, const AxisEntry &X, int k, int lane,
+                                              int &r, int &c, int &word)
+{
+    const int ncl = X.R - X.A;
+    const int line = k >> 1, pos = ((k & 1) << 5) + lane;
+    if (line < ncl) {
+        c = X.A + line; r = Y.L + pos;
+        word = mbox_col_word(r, c);
+        return r < Y.R;
+    }
+    r = Y.A + (line - ncl); c = X.L + pos;
+    word = mbox_row_word(r, c);
+    return r < Y.R && c < X.A;
+}
+__device__ __forceinline__ int arrival_chunks(const AxisEntry &Y, const AxisEntry &X)
+{
+    if (Y.R <= Y.L || X.R <= X.L) return 0;
+    return 2 * ((X.R - X.A) + (X.A > X.L ? Y.R - Y.A : 0));
+}
+
+template <int WQ>
 __global__ void __launch_bounds__(CV_NT, 1)
 conveyor_kernel(const __grid_constant__ CParams p)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
     Smem &sm = *reinterpret_cast<Smem *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int cta = blockIdx.x;
@@ -238,14 +422,6 @@ conveyor_kernel(const __grid_constant__ CParams p)
     const int t2 = cta - bl * p.NR * p.NC;
     const int ci = t2 / p.NC, cj = t2 - ci * p.NC;
     const size_t frame_off = (size_t)(p.frame0 + bl) * p.H * p.W;
-    const size_t frame_off_q = (size_t)(p.frame0 + bl) * p.H * p.Wq;
-    const size_t plane = (size_t)p.B_total * p.H * p.Wq;
-    // receivers of departing pixels: bit 0 = left neighbour, bit 1 = upper neighbour (3 = up-left)
-    const int cjl = (cj + p.NC - 1) % p.NC, ciu = (ci + p.NR - 1) % p.NR;
-    auto nbr_cta = [&](int which) {
-        return (bl * p.NR + ((which & 2) ? ciu : ci)) * p.NC + ((which & 1) ? cjl : cj);
-    };
-    unsigned long long *my_box = p.mbox + (size_t)cta * CV_D * CV_MBW;
     const int total = p.total;
 
     // ---- prologue: families and the first table entries into shared memory; x <- y on the tile ----
@@ -254,6 +430,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
         const int g = i >> 1, ax = i & 1;
         sm.tab[g % CV_TR][ax] = ax ? p.tabx[(size_t)g * p.NC + cj] : p.taby[(size_t)g * p.NR + ci];
     }
+    if (tid == 0) sm.abort = 0;
     __syncthreads();
     {
         const AxisEntry ey = sm.tab[0][0], ex = sm.tab[0][1];
@@ -263,61 +440,58 @@ conveyor_kernel(const __grid_constant__ CParams p)
             sm.xs[tidx(r, c)] = p.y[frame_off + (size_t)r * p.W + c];
         }
     }
+    ControlState cs;                            // control lane only
+    cs.geom = 0; cs.key = -1; cs.phase = 0;
+    const unsigned long long frame_off_q = (unsigned long long)(p.frame0 + bl) * p.H * p.Wq;
+    const unsigned long long plane = (unsigned long long)p.B_total * p.H * p.Wq;
+    if (tid == CV_NCW * 32) {
+        for (int i = 0; i < CV_NST; ++i) mbar_init(&sm.qbar[i], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        cs.plane_f = frame_off_q;
+        make_desc(sm, p, cs, 0, 0, 0, total);
+    }
     __syncthreads();
 
-    // role state (each used by one warp only)
-    unsigned long long pend0 = 0, pend1 = 0;   // receiver: mailbox words loaded one step ahead
-    unsigned prog_pend = 0, prog_seen = 0;     // sender lanes 1..3: progress of the receiving CTAs
-    int prog_iter = -1;                        // step at which prog_pend was requested (-1: none in flight)
-    int status_pend = 0;                       // receiver lane 0: the failure flag, loaded one step ahead
-    int f = 0;                                 // family of step g
-    int fp = CV_PF % p.F;                      // family of step g + CV_PF
-
-    for (int g = 0; g < total; ++g) {
-        int bad = 0;
-        if (warp < CV_NCW) {
-            // ---- compute warps: the windows of step g ---------------------------------------------------
-            const AxisEntry ey = sm.tab[g % CV_TR][0], ex = sm.tab[g % CV_TR][1];
-            if (ey.nw > 0 && ex.nw > 0) {
-                const CFamily fam = sm.fams[f];
-                float *qplane = p.q + (size_t)f * plane + frame_off_q;
-                const float *qst = sm.qs[g % CV_NST];
-                const bool first = g < p.F;
-                switch (fam.side) {
-                    case 1: project_tile<1, 8>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
-                    case 2: project_tile<2, 4>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
-                    case 3: project_tile<3, 3>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
-                    case 4: project_tile<4, 2>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
-                    case 5: project_tile<5, 2>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
-                    case 6: project_tile<6, 1>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
-                    case 7: project_tile<7, 1>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
-                    case 8: project_tile<8, 1>(sm, qst, qplane, ey, ex, fam.c, fam.sqrt_c, p.Wq, first, warp, lane); break;
-                    default:
-                        if (fam.G <= 16) project_tile_big<16>(sm, qst, qplane, ey, ex, fam.side, fam.c, fam.sqrt_c, p.Wq, first, warp, lane);
-                        else project_tile_big<32>(sm, qst, qplane, ey, ex, fam.side, fam.c, fam.sqrt_c, p.Wq, first, warp, lane);
-                }
+    if (warp < CV_NCW) {
+        // =============== compute warps: runs of steps with one window edge ===============================
+        LaneCache lc;
+        lc.geom = -1; lc.nwin = 0; lc.rr0 = lc.colofs = lc.lq = lc.lg = 0;
+        int g = 0;
+        while (g < total) {
+            const int f = sm.desc[g & 1].f;
+            const int g_end = g + sm.desc[g & 1].run_left;
+            const CFamily fam = sm.fams[f];
+            switch (fam.side) {
+                case 1: run_steps<1, cv_kr(1), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
+                case 2: run_steps<2, cv_kr(2), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
+                case 3: run_steps<3, cv_kr(3), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
+                case 4: run_steps<4, cv_kr(4), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
+                case 5: run_steps<5, cv_kr(5), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
+                case 6: run_steps<6, cv_kr(6), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
+                case 7: run_steps<7, cv_kr(7), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
+                case 8: run_steps<8, cv_kr(8), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
+                default:
+                    if (fam.side <= 16) run_steps_big<16, WQ>(sm, p, fam.side, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total);
+                    else run_steps_big<32, WQ>(sm, p, fam.side, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total);
             }
-        } else if (warp == CV_NCW) {
-            // ---- loader warp: q of step g + CV_PF and the table entry of step g + CV_LA + 1 ---------------
-            const int gp = g + CV_PF;
-            if (gp < total && gp >= p.F) {                           // the first sweep reads no q (q = 0)
-                const AxisEntry qy = sm.tab[gp % CV_TR][0], qx = sm.tab[gp % CV_TR][1];
-                if (qy.nw > 0 && qx.nw > 0) {
-                    const int s = sm.fams[fp].side;
-                    const int rows = qy.nw * s;
-                    const int c0 = qx.w0 & ~3, c1 = (qx.w0 + qx.nw * s + 3) & ~3;
-                    const int half = lane >> 4, ch = lane & 15;      // 16 chunks of 4 columns cover a row
-                    const int c = c0 + 4 * ch;
-                    if (c < c1 && c < p.Wq) {
-                        const float *src = p.q + (size_t)fp * plane + frame_off_q + (size_t)(qy.w0 + half) * p.Wq + c;
-                        unsigned dst = (unsigned)__cvta_generic_to_shared(sm.qs[gp % CV_NST]) + 4u * (unsigned)(half * CV_PW + 4 * ch);
-                        for (int rr = half; rr < rows; rr += 2) {
-                            cp_async16(dst, src);
-                            dst += 2 * CV_PW * 4;
-                            src += 2 * (size_t)p.Wq;
-                        }
-                    }
-                }
+            if (g < g_end) return;                                   // a run was cut short: abort
+        }
+    } else if (warp == CV_NCW) {
+        // =============== control warp: q boxes by TMA, table prefetch, next step's descriptor ============
+        int f1 = 1 % p.F;                      // family of step g + 1
+        int fp = CV_PF % p.F;                  // family of step g + CV_PF
+        int st1 = 1 % CV_NST;                  // q stage of step g + 1
+        int stp = CV_PF % CV_NST;              // q stage of step g + CV_PF
+        if (lane == 0) {
+            cs.plane_f = frame_off_q + (unsigned long long)f1 * plane;
+            cs.row_fp = (fp * p.B_total + p.frame0 + bl) * p.H;
+        }
+        for (int g = 0; g < total; ++g) {
+            if (lane == 0 && step_loads_q(sm, p, g + CV_PF, total)) {      // the q box of step g + CV_PF
+                const AxisEntry qy = sm.tab[(g + CV_PF) % CV_TR][0], qx = sm.tab[(g + CV_PF) % CV_TR][1];
+                const int k = (qy.e1 + 7) >> 3;                              // box of 8k rows, qp columns
+                mbar_expect_tx(&sm.qbar[stp], (unsigned)(k * 8 * p.qp * 4));
+                tma_load_2d(sm.qs + (size_t)stp * (CV_PW * CV_PW), &p.qmap[k - 1], qx.e0, cs.row_fp + qy.w0, &sm.qbar[stp]);  // column: 16-byte aligned
             }
             const int gt = g + CV_LA + 1;
             if (gt < total && lane < 2) {
@@ -325,99 +499,117 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 cp_async16((unsigned)__cvta_generic_to_shared(&sm.tab[gt % CV_TR][lane]), src);
             }
             cp_async_commit();
-            cp_async_wait<CV_PF - 1>();                              // q of step g+1 has landed
-        } else if (warp == CV_NCW + 1) {
-            // ---- sender warp: departures of step g-1 -> the neighbours' mailboxes, tagged g --------------
+            if (lane == 0) CV_STAMP(7);
+            if (lane == 0 && g + 1 < total) make_desc(sm, p, cs, g + 1, f1, st1, total);
+            cp_async_wait<CV_PF - 1>();
+            if (lane == 0 && step_loads_q(sm, p, g + 1, total)) {            // q of step g+1 has landed
+                const unsigned parity = (cs.phase >> st1) & 1u;
+                const long long t0 = clock64();
+                while (!mbar_try_wait(&sm.qbar[st1], parity))
+                    if (clock64() - t0 > 2000000000LL) { atomicExch(p.status, 1); break; }
+                cs.phase ^= 1u << st1;
+            }
+            if (lane == 0) CV_STAMP(3);
+            CV_STEP_BARRIER();
+            if (++f1 == p.F) { f1 = 0; cs.plane_f = frame_off_q; } else cs.plane_f += plane;
+            if (++fp == p.F) { fp = 0; cs.row_fp = (p.frame0 + bl) * p.H; } else cs.row_fp += p.B_total * p.H;
+            if (++st1 == CV_NST) st1 = 0;
+            if (++stp == CV_NST) stp = 0;
+        }
+    } else if (warp == CV_NCW + 1) {
+        // =============== sender warp: departures of step g-1 -> the neighbours' mailboxes, tagged g ======
+        // receivers of departing pixels: bit 0 = left neighbour, bit 1 = upper neighbour (3 = up-left)
+        const int cjl = (cj + p.NC - 1) % p.NC, ciu = (ci + p.NR - 1) % p.NR;
+        auto nbr_cta = [&](int which) {
+            return (bl * p.NR + ((which & 2) ? ciu : ci)) * p.NC + ((which & 1) ? cjl : cj);
+        };
+        unsigned long long *const box_l = p.mbox + (size_t)nbr_cta(1) * CV_D * CV_MBW;
+        unsigned long long *const box_u = p.mbox + (size_t)nbr_cta(2) * CV_D * CV_MBW;
+        unsigned long long *const box_ul = p.mbox + (size_t)nbr_cta(3) * CV_D * CV_MBW;
+        const unsigned *my_nbr_prog = p.prog + (size_t)nbr_cta(lane >= 1 && lane <= 3 ? lane : 1) * CV_PROG_STRIDE;
+        unsigned prog_pend = 0, prog_seen = 0;  // lanes 1..3: progress of the receiving CTAs
+        int prog_iter = -1;                     // step at which prog_pend was requested (-1: none in flight)
+        for (int g = 0; g < total; ++g) {
             if (g > 0) {
                 if (lane >= 1 && lane <= 3) {                        // the ring slot must have been read
                     // the neighbour's counter is re-read only when the ring is half used, and the value is
                     // picked up a few steps later: the load must never sit on this warp's critical path
                     if (prog_iter >= 0 && g >= prog_iter + 3) { prog_seen = max(prog_seen, prog_pend); prog_iter = -1; }
                     if ((int)prog_seen + CV_D < g) {
-                        prog_seen = poll_prog(p.prog + (size_t)nbr_cta(lane) * CV_PROG_STRIDE, (unsigned)(g - CV_D), p.status);
+                        prog_seen = poll_prog(my_nbr_prog, (unsigned)(g - CV_D), p.status);
                         prog_iter = -1;
                     } else if (prog_iter < 0 && (int)prog_seen + CV_D / 2 < g) {
-                        prog_pend = ld_u32_gpu(p.prog + (size_t)nbr_cta(lane) * CV_PROG_STRIDE);
+                        prog_pend = ld_u32_gpu(my_nbr_prog);
                         prog_iter = g;
                     }
                 }
                 __syncwarp();
-                if (p.trace && lane == 0) {
-                    unsigned long long t;
-                    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-                    p.trace[((size_t)cta * total + g) * 8 + 6] = t;
-                }
                 const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
-                const size_t slot = (size_t)(g % CV_D) * CV_MBW;
+                const int slot = (g % CV_D) * CV_MBW;
                 const unsigned long long tag = (unsigned long long)(unsigned)g << 32;
                 for (int c = px.L; c < px.D; ++c)                    // column strip: columns [L, D), all rows
                     for (int r = py.L + lane; r < py.R; r += 32) {
-                        const int which = 1 | (r < py.D ? 2 : 0);
-                        st_u64_gpu(p.mbox + (size_t)nbr_cta(which) * CV_D * CV_MBW + slot + mbox_col_word(r, c),
-                                   tag | __float_as_uint(sm.xs[tidx(r, c)]));
+                        unsigned long long *box = (r < py.D) ? box_ul : box_l;
+                        st_u64_gpu(box + slot + mbox_col_word(r, c), tag | __float_as_uint(sm.xs[tidx(r, c)]));
                     }
                 for (int r = py.L; r < py.D; ++r)                    // row strip: rows [L, D), columns [D, R)
                     for (int c = px.D + lane; c < px.R; c += 32)
-                        st_u64_gpu(p.mbox + (size_t)nbr_cta(2) * CV_D * CV_MBW + slot + mbox_row_word(r, c),
-                                   tag | __float_as_uint(sm.xs[tidx(r, c)]));
+                        st_u64_gpu(box_u + slot + mbox_row_word(r, c), tag | __float_as_uint(sm.xs[tidx(r, c)]));
             }
-        } else {
-            // ---- receiver warp: arrivals of step g+1 into the tile; preload the first line of step g+2 ----
+            if (lane == 0) CV_STAMP(4);
+            CV_STEP_BARRIER();
+        }
+    } else {
+        // =============== receiver warp: arrivals of step g+1 into the tile ================================
+        unsigned long long *const my_box = p.mbox + (size_t)cta * CV_D * CV_MBW;
+        unsigned long long pend[4] = {0, 0, 0, 0};   // the first four chunks of step g+2, loaded a step ahead
+        int status_pend = 0;                         // lane 0: the failure flag, loaded a step ahead
+        for (int g = 0; g < total; ++g) {
             if (g + 1 < total) {
                 const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
                 const unsigned long long *box = my_box + (size_t)((g + 1) % CV_D) * CV_MBW;
                 const unsigned tag = (unsigned)(g + 1);
-                bool first_line = true;
-                for (int c = nx.A; c < nx.R; ++c) {                  // column strip: columns [A, R), all rows
-                    for (int r = ny.L + lane, t = 0; r < ny.R; r += 32, ++t) {
-                        unsigned long long wv = (first_line && t < 2) ? (t ? pend1 : pend0) : 0ull;
-                        if ((unsigned)(wv >> 32) != tag) wv = poll_tag(box + mbox_col_word(r, c), tag, p.status);
-                        sm.xs[tidx(r, c)] = __uint_as_float((unsigned)wv);
+                const int nchunks = arrival_chunks(ny, nx);
+                for (int k0 = 0; k0 < nchunks; k0 += 4) {
+                    unsigned long long w[4];
+                    int xi[4], wd[4];
+                    bool ok[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        int r, c;
+                        ok[u] = (k0 + u < nchunks) && arrival_chunk(ny, nx, k0 + u, lane, r, c, wd[u]);
+                        xi[u] = tidx(r, c);
+                        w[u] = (k0 == 0) ? pend[u] : (ok[u] ? ld_u64_gpu(box + wd[u]) : 0ull);
                     }
-                    first_line = false;
-                }
-                for (int r = ny.A; r < ny.R; ++r) {                  // row strip: rows [A, R), columns [L, A)
-                    for (int c = nx.L + lane, t = 0; c < nx.A; c += 32, ++t) {
-                        unsigned long long wv = (first_line && t < 2) ? (t ? pend1 : pend0) : 0ull;
-                        if ((unsigned)(wv >> 32) != tag) wv = poll_tag(box + mbox_row_word(r, c), tag, p.status);
-                        sm.xs[tidx(r, c)] = __uint_as_float((unsigned)wv);
-                    }
-                    first_line = false;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (ok[u]) {
+                            if ((unsigned)(w[u] >> 32) != tag) w[u] = poll_tag(box + wd[u], tag, p.status);
+                            sm.xs[xi[u]] = __uint_as_float((unsigned)w[u]);
+                        }
                 }
                 __syncwarp();
-                if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // mailbox of step g+1 has been read
-                pend0 = pend1 = 0;
+                if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // step g+1 has been read
+#pragma unroll
+                for (int u = 0; u < 4; ++u) pend[u] = 0;
                 if (g + 2 < total) {
                     const AxisEntry my = sm.tab[(g + 2) % CV_TR][0], mx = sm.tab[(g + 2) % CV_TR][1];
                     const unsigned long long *box2 = my_box + (size_t)((g + 2) % CV_D) * CV_MBW;
-                    if (mx.A < mx.R) {                               // first line = first arriving column
-                        const int r = my.L + lane;
-                        if (r < my.R) pend0 = ld_u64_gpu(box2 + mbox_col_word(r, mx.A));
-                        if (r + 32 < my.R) pend1 = ld_u64_gpu(box2 + mbox_col_word(r + 32, mx.A));
-                    } else if (my.A < my.R) {                        // ... or the first arriving row
-                        const int c = mx.L + lane;
-                        if (c < mx.A) pend0 = ld_u64_gpu(box2 + mbox_row_word(my.A, c));
-                        if (c + 32 < mx.A) pend1 = ld_u64_gpu(box2 + mbox_row_word(my.A, c + 32));
+                    const int mchunks = arrival_chunks(my, mx);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        int r, c, wd;
+                        if (u < mchunks && arrival_chunk(my, mx, u, lane, r, c, wd)) pend[u] = ld_u64_gpu(box2 + wd);
                     }
                 }
             }
-            if (lane == 0) { bad = status_pend; status_pend = *(volatile int *)p.status; }
+            if (lane == 0 && (g & 7) == 3) {
+                if (status_pend) sm.abort = 1;
+                status_pend = *(volatile int *)p.status;             // consumed 8 steps later
+            }
+            if (lane == 0) CV_STAMP(5);
+            CV_STEP_BARRIER();
         }
-
-        // ---- one barrier per step ----------------------------------------------------------------------
-        if (p.trace && lane == 0 && (warp == 0 || warp >= CV_NCW - 1)) {      // debug: when each role finished
-            unsigned long long t;
-            asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-            p.trace[((size_t)cta * total + g) * 8 + 1 + (warp == 0 ? 0 : warp - (CV_NCW - 2))] = t;
-        }
-        if (__syncthreads_or(bad)) return;
-        if (p.trace && tid == 0) {
-            unsigned long long t;
-            asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-            p.trace[((size_t)cta * total + g) * 8] = t;
-        }
-        if (++f == p.F) f = 0;
-        if (++fp == p.F) fp = 0;
     }
 
     // ---- a9: x_out <- the tile of the last step -----------------------------------------------------
@@ -428,6 +620,17 @@ conveyor_kernel(const __grid_constant__ CParams p)
             const int r = ey.L + i / w, c = ex.L + i % w;
             p.x_out[frame_off + (size_t)r * p.W + c] = sm.xs[tidx(r, c)];
         }
+    }
+}
+
+using ConveyorKernel = void (*)(const CParams);
+// q row pitches with their own instantiation (immediate row offsets in the q stores); 0 = run-time pitch
+static ConveyorKernel kernel_for(int Wq)
+{
+    switch (Wq) {
+        case 512: return conveyor_kernel<512>;
+        case 256: return conveyor_kernel<256>;
+        default: return conveyor_kernel<0>;
     }
 }
 
@@ -442,6 +645,9 @@ struct ConveyorPlan {
     int H, W, Wq, B, F;
     int T_y, T_x, NR, NC;
     int frames_per_launch;
+    ConveyorKernel kernel;
+    int qp = 0;                         // columns of a TMA box = row pitch of a q stage
+    CUtensorMap qmap[8];
     std::vector<Family> fams;
     float *q, *xwork;
     CFamily *d_fams = nullptr;
@@ -488,18 +694,22 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
                                    float *xwork)
 {
     if (fams.empty() || (int)fams.size() > CV_MAX_F || H > 32000 || W > 32000) return nullptr;
+    // q of a step is fetched CV_PF steps ahead of its use and was written one sweep (F steps) earlier
+    if ((int)fams.size() < CV_PF + 3) return nullptr;
+    if ((long long)fams.size() * B * H >= (1ll << 31)) return nullptr;          // tensor rows are 32-bit coordinates
     int dev = 0, n_sm = 0, smem_optin = 0, coop = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
     if (!coop || (size_t)smem_optin < sizeof(Smem)) return nullptr;
-    if (cudaFuncSetAttribute(conveyor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)) != cudaSuccess) {
+    const ConveyorKernel kernel = kernel_for((W + 3) & ~3);
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)) != cudaSuccess) {
         cudaGetLastError();
         return nullptr;
     }
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, conveyor_kernel, CV_NT, sizeof(Smem)) != cudaSuccess || per_sm < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, CV_NT, sizeof(Smem)) != cudaSuccess || per_sm < 1) {
         cudaGetLastError();
         return nullptr;
     }
@@ -512,14 +722,41 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
     ConveyorPlan *pl = new ConveyorPlan;
     pl->H = H; pl->W = W; pl->Wq = (W + 3) & ~3; pl->B = B; pl->F = (int)fams.size();
     pl->T_y = cs.T_y; pl->T_x = cs.T_x; pl->NR = cs.tiles_y; pl->NC = cs.tiles_x;
-    pl->fams = fams; pl->q = q; pl->xwork = xwork;
+    pl->fams = fams; pl->q = q; pl->xwork = xwork; pl->kernel = kernel;
+    {   // q as a 2-D fp32 tensor [F*B*H][Wq]; one map per box height 8, 16, .., 64 (plain layout, zero fill)
+        typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+            cudaGetLastError();
+            delete pl;
+            return nullptr;
+        }
+        pl->qp = std::min(CV_PW, pl->Wq);
+        const cuuint64_t gdim[2] = {(cuuint64_t)pl->Wq, (cuuint64_t)fams.size() * B * H};
+        const cuuint64_t gstride[1] = {(cuuint64_t)pl->Wq * sizeof(float)};
+        const cuuint32_t estr[2] = {1, 1};
+        for (int k = 0; k < 8; ++k) {
+            const cuuint32_t box[2] = {(cuuint32_t)pl->qp, (cuuint32_t)(8 * (k + 1))};
+            if (((EncodeFn)fn)(&pl->qmap[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, q, gdim, gstride, box, estr,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                               CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+                delete pl;
+                return nullptr;
+            }
+        }
+    }
     const int tiles = pl->NR * pl->NC;
     pl->frames_per_launch = std::max(1, std::min(B, capacity / tiles));
     std::vector<CFamily> cf(fams.size());
     for (size_t i = 0; i < fams.size(); ++i) {
-        int G = 1;
-        while (G < fams[i].side) G <<= 1;
-        cf[i] = CFamily{fams[i].side, G, fams[i].c, fams[i].sqrt_c};
+        int lg = 0;
+        while ((1 << lg) < fams[i].side) ++lg;
+        size_t e = i;
+        while (e + 1 < fams.size() && fams[e + 1].side == fams[i].side) ++e;
+        cf[i] = CFamily{fams[i].side, lg, (int)(e - i + 1), 0, fams[i].c, fams[i].sqrt_c, {0, 0}};
     }
     const size_t n_cta = (size_t)pl->frames_per_launch * tiles;
     pl->mbox_bytes = n_cta * CV_D * CV_MBW * sizeof(unsigned long long);
@@ -577,7 +814,8 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
     p.y = y; p.x_out = x_out; p.q = pl->q; p.fams = pl->d_fams; p.taby = tabs->d_y; p.tabx = tabs->d_x;
     p.mbox = pl->d_mbox; p.prog = pl->d_prog; p.status = pl->d_status;
     p.F = pl->F; p.total = pl->F * n_sweeps; p.H = pl->H; p.W = pl->W; p.Wq = pl->Wq; p.B_total = pl->B;
-    p.NR = pl->NR; p.NC = pl->NC;
+    p.NR = pl->NR; p.NC = pl->NC; p.qp = pl->qp;
+    memcpy(p.qmap, pl->qmap, sizeof p.qmap);
     const int tiles = pl->NR * pl->NC;
     const char *trace_path = getenv("SMRE_CV_TRACE");        // debug only: synchronises and writes a file
     if (trace_path && cudaMalloc(&p.trace, (size_t)tiles * p.total * 64) != cudaSuccess) p.trace = nullptr;
@@ -588,7 +826,7 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
         if ((e = cudaMemsetAsync(pl->d_mbox, 0, (size_t)nb * tiles * CV_D * CV_MBW * 8, st)) != cudaSuccess) return e;
         if ((e = cudaMemsetAsync(pl->d_prog, 0, (size_t)nb * tiles * CV_PROG_STRIDE * sizeof(unsigned), st)) != cudaSuccess) return e;
         void *args[] = {&p};
-        e = cudaLaunchCooperativeKernel((const void *)conveyor_kernel, dim3((unsigned)(nb * tiles)),
+        e = cudaLaunchCooperativeKernel((const void *)pl->kernel, dim3((unsigned)(nb * tiles)),
                                         dim3(CV_NT), args, sizeof(Smem), st);
         if (e != cudaSuccess) return e;
         if (launches) ++*launches;

@@ -10,7 +10,7 @@
 namespace smre {
 
 constexpr int CV_NCW = 16;              // compute warps per CTA
-constexpr int CV_NT = (CV_NCW + 3) * 32;    // + one loader, one sender, one receiver warp
+constexpr int CV_NT = (CV_NCW + 3) * 32;    // + one control, one sender, one receiver warp
 constexpr int CV_PW = 64;               // edge of the torus-addressed x tile in shared memory
 constexpr int CV_SD = 16;               // strip depth: a boundary moves < CV_SD pixels per step
 constexpr int CV_D = 16;                // mailbox ring depth (steps)
@@ -28,8 +28,13 @@ struct AxisEntry {
     short A;           // pixels [A, R) were not held after the previous step: they ARRIVE
     short D;           // pixels [L, D) are not held at the next step: they DEPART after this step
     short w0, nw;      // windows of this step's family with origin in [L, R): first origin, count
-    unsigned magic;    // floor(n / nw) == (n * magic) >> 20 for n < 2^12   (nw >= 1)
+    short e0, e1;      // y axis: blocks of cv_kr(side) window rows, rows of the window box (nw * side)
+                       // x axis: first 4-aligned column c0 of the q box, 16-byte chunks per row of it
 };
+
+// Vertically stacked windows handled by one lane of the conveyor kernel, per window edge (the kernel's
+// template instantiations and the planner's e0 must agree on this).
+__host__ __device__ constexpr int cv_kr(int side) { return side == 1 ? 8 : side == 2 ? 4 : side == 3 ? 3 : side <= 5 ? 2 : 1; }
 static_assert(sizeof(AxisEntry) == 16, "AxisEntry must be 16 bytes");
 
 // Tile-boundary trajectories of one axis for `total` steps.

@@ -29,7 +29,20 @@ static void set_why(char *why, size_t n, const char *fmt, int a = 0, int b = 0, 
     if (why && n) snprintf(why, n, fmt, a, b, c);
 }
 
-static unsigned magic20(int d) { return d > 0 ? (unsigned)(((1u << 20) + d - 1) / d) : 0u; }
+// extra per-axis numbers the kernel would otherwise derive every step
+static void fill_extras(AxisEntry &e, bool y_axis, int s, int N)
+{
+    if (y_axis) {
+        const int kr = cv_kr(s);
+        e.e0 = (short)((e.nw + kr - 1) / kr);
+        e.e1 = (short)(e.nw * s);
+    } else {
+        const int pitch = (N + 3) & ~3;                       // row pitch of the q planes
+        const int c0 = e.w0 & ~3, c1 = std::min((e.w0 + e.nw * s + 3) & ~3, pitch);
+        e.e0 = (short)c0;
+        e.e1 = (short)(e.nw > 0 ? (c1 - c0) >> 2 : 0);
+    }
+}
 
 static void window_range(int L, int R, int s, int o, int N, short &w0, short &nw)
 {
@@ -61,7 +74,7 @@ bool plan_axis(int N, const std::vector<Family> &fams, bool y_axis, int n_sweeps
             AxisEntry e{};
             e.L = 0; e.R = (short)N; e.A = (short)(g == 0 ? 0 : N); e.D = 0;
             window_range(0, N, side(g), off(g), N, e.w0, e.nw);
-            e.magic = magic20(e.nw);
+            fill_extras(e, y_axis, side(g), N);
             out.tab[g] = e;
         }
         return true;
@@ -120,7 +133,7 @@ bool plan_axis(int N, const std::vector<Family> &fams, bool y_axis, int n_sweeps
             }
             e.A = (short)A; e.D = (short)D;
             window_range(L, R, s, o, N, e.w0, e.nw);
-            e.magic = magic20(e.nw);
+            fill_extras(e, y_axis, s, N);
             const int slot = ((k % S) + S) % S;
             AxisEntry &dst = out.tab[(size_t)g * S + slot];
             if (dst.R > dst.L) { set_why(why, why_len, "two live tiles in slot %d at step %d", slot, g); return false; }
