@@ -139,7 +139,7 @@ static_assert(CV_PW == 64, "tidx assumes a 64 x 64 torus");
 __device__ __forceinline__ int mbox_col_word(int r, int c) { return ((c & (CV_SD - 1)) << 6) | (r & 63); }
 __device__ __forceinline__ int mbox_row_word(int r, int c) { return CV_SD * 64 + (((r & (CV_SD - 1)) << 6) | (c & 63)); }
 
-// Per-step descriptor (32 bytes = two 16-byte broadcast loads), written one step ahead by the control
+// Per-step descriptor (48 bytes; the compute warps read the first 32), written one step ahead by the control
 // warp so that the compute warps do almost no index arithmetic of their own.
 struct StepDesc {
     // v0
@@ -152,8 +152,12 @@ struct StepDesc {
     unsigned goff_lo, goff_hi;    // element offset in q of (family plane, frame, first window row, first window column)
     int f;                        // family index of this step
     int run_left;                 // steps left in this run of equal window edges, this one included
+    // v2: the TMA box that brings this step's q (issued CV_PF steps before the step, awaited just before it)
+    int tma_col, tma_row;         // tensor coordinates: 4-aligned column, row of (family, frame, first window row)
+    int tma_k;                    // box height / 8 (1..8); 0: this step reads no q
+    int pad;
 };
-static_assert(sizeof(StepDesc) == 32, "StepDesc must be 32 bytes");
+static_assert(sizeof(StepDesc) == 48, "StepDesc must be 48 bytes");
 
 struct GeomDesc { int nwx, nwy, n_items, pad; };   // read by the lanes only when StepDesc::geom changes
 
@@ -161,8 +165,8 @@ struct Smem {
     float xs[CV_PW * CV_PW];                 // the x tile, torus addressed by image (row, column)
     float qs[CV_NST * CV_PW * CV_PW];        // q stages, filled by TMA: [(row - first window row) * qp + (column - c0)], c0 = first window column rounded down to 4
     AxisEntry tab[CV_TR][2];                 // [step % CV_TR][0 = y, 1 = x]
-    StepDesc desc[2];                        // [step & 1]
-    GeomDesc geo[2];                         // [geom & 1]
+    StepDesc desc[CV_DR];                    // [step % CV_DR]
+    GeomDesc geo[16];                        // [geom & 15]
     unsigned long long qbar[CV_NST];         // mbarriers: the TMA box of a stage has landed
     CFamily fams[CV_MAX_F];
     int abort;                               // set by the receiver warp when the failure flag is up
@@ -298,10 +302,10 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
     const int Wq = WQ ? WQ : p.Wq;
     const int qp = WQ ? CV_PW : p.qp;
     for (; g < g_end; ++g) {
-        const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g & 1].geom);
+        const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g % CV_DR].geom);
         if (warp == 0 && lane == 0) CV_STAMP(6);
         if ((int)v0.x != lc.geom) {                            // rare: the tile's window counts changed
-            const GeomDesc ge = sm.geo[v0.x & 1];
+            const GeomDesc ge = sm.geo[v0.x & 15];
             const int n_items = (int)v0.y;
             lc.geom = (int)v0.x;
             const int item = warp * 32 + lane;
@@ -316,13 +320,13 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
             lc.lg = lc.rr0 * Wq + lc.colofs;
         }
         if (lc.busy) {
-            const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g & 1].goff_lo);
+            const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g % CV_DR].goff_lo);
             const int r0 = (int)(v0.z & 0xffffu) + lc.rr0, cc = (int)(v0.z >> 16) + lc.colofs;
             const float *qs0 = sm.qs + (v0.w & 0x7fffffffu) + lc.lq;
             float *qg = p.q + (((unsigned long long)v1.y << 32) | v1.x) + lc.lg;
             project_item<S, KR, G, WQ>(sm.xs, qs0, qg, tidx(r0, cc), lc.nwin, c, sqrt_c, p.Wq, p.qp, (v0.w >> 31) != 0);
             if ((int)v0.y > CV_NCW * 32)
-                project_generic<G>(sm, sm.geo[v0.x & 1], S, KR, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
+                project_generic<G>(sm, sm.geo[v0.x & 15], S, KR, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
                                    sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
                                    c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, CV_NCW * 32, warp, lane);
         }
@@ -341,50 +345,75 @@ __device__ __forceinline__ void run_steps_big(Smem &sm, const CParams &p, int s,
     const int Wq = WQ ? WQ : p.Wq;
     const int qp = WQ ? CV_PW : p.qp;
     for (; g < g_end; ++g) {
-        const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g & 1].geom);
-        const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g & 1].goff_lo);
+        const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g % CV_DR].geom);
+        const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g % CV_DR].goff_lo);
         if ((int)v0.y > 0)
-            project_generic<G>(sm, sm.geo[v0.x & 1], s, 1, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
+            project_generic<G>(sm, sm.geo[v0.x & 15], s, 1, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
                                sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
                                c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, 0, warp, lane);
         CV_STEP_BARRIER();
     }
 }
 
-// Control lane: the descriptor of step g (family f, q stage st = g % CV_NST).
-struct ControlState {
-    int geom, key;                     // geometry id and what it stands for
-    unsigned long long plane_f;        // f * plane + frame offset (elements)
-    int row_fp;                        // tensor row of (family fp, frame, row 0): (fp * B_total + frame) * H
-    unsigned phase;                    // bit s: parity the next wait on q stage s has to use
-};
-__device__ __forceinline__ void make_desc(Smem &sm, const CParams &p, ControlState &cs, int g, int f, int st,
-                                          int total)
+// Control warp, all lanes: lane i plans step first + i (i < count <= 32) into the descriptor ring.
+// geom / key: geometry id and key of the last step planned before `first` (warp-uniform, updated).
+__device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first, int count, int lane, int total,
+                                           unsigned long long frame_off_q, unsigned long long plane, int frame,
+                                           int &geom, int &key)
 {
-    const AxisEntry ey = sm.tab[g % CV_TR][0], ex = sm.tab[g % CV_TR][1];
-    const CFamily fam = sm.fams[f];
-    StepDesc d;
-    const int n_items = (ey.nw > 0 && ex.nw > 0) ? (ey.e0 * ex.nw) << fam.lgG : 0;
-    const int key = (fam.side << 16) | (ey.nw << 8) | ex.nw;
-    if (key != cs.key) {
-        cs.key = key; ++cs.geom;
-        GeomDesc ge; ge.nwx = ex.nw; ge.nwy = ey.nw; ge.n_items = n_items; ge.pad = 0;
-        sm.geo[cs.geom & 1] = ge;
+    const int g = first + lane;
+    const bool on = lane < count && g < total;
+    int my_key = key, n_items = 0;
+    AxisEntry ey{}, ex{};
+    CFamily fam{};
+    int f = 0;
+    if (on) {
+        ey = sm.tab[g % CV_TR][0]; ex = sm.tab[g % CV_TR][1];
+        f = g % p.F;
+        fam = sm.fams[f];
+        n_items = (ey.nw > 0 && ex.nw > 0) ? (ey.e0 * ex.nw) << fam.lgG : 0;
+        my_key = (fam.side << 16) | (ey.nw << 8) | ex.nw;
     }
-    d.geom = cs.geom; d.n_items = n_items;
-    d.w0yx = ey.w0 | (ex.w0 << 16);
-    d.qbase = (unsigned)(st * (CV_PW * CV_PW) + (ex.w0 - ex.e0)) | (g < p.F ? 0x80000000u : 0u);
-    const unsigned long long goff = cs.plane_f + (unsigned)(ey.w0 * p.Wq + ex.w0);
-    d.goff_lo = (unsigned)goff; d.goff_hi = (unsigned)(goff >> 32);
-    d.f = f; d.run_left = min(fam.run_left, total - g);
-    sm.desc[g & 1] = d;
+    // geometry ids: a new id wherever the key differs from the previous step's
+    int prev_key = __shfl_up_sync(0xffffffffu, my_key, 1);
+    if (lane == 0) prev_key = key;
+    const bool changed = on && my_key != prev_key;
+    const unsigned chg = __ballot_sync(0xffffffffu, changed);
+    const int my_geom = geom + __popc(chg & (0xffffffffu >> (31 - lane)));
+    if (changed) {
+        GeomDesc ge; ge.nwx = ex.nw; ge.nwy = ey.nw; ge.n_items = n_items; ge.pad = 0;
+        sm.geo[my_geom & 15] = ge;
+    }
+    if (on) {
+        StepDesc d;
+        d.geom = my_geom; d.n_items = n_items;
+        d.w0yx = ey.w0 | (ex.w0 << 16);
+        d.qbase = (unsigned)((g % CV_NST) * (CV_PW * CV_PW) + (ex.w0 - ex.e0)) | (g < p.F ? 0x80000000u : 0u);
+        const unsigned long long goff = frame_off_q + (unsigned long long)f * plane + (unsigned)(ey.w0 * p.Wq + ex.w0);
+        d.goff_lo = (unsigned)goff; d.goff_hi = (unsigned)(goff >> 32);
+        d.f = f; d.run_left = min(fam.run_left, total - g);
+        d.tma_col = ex.e0;
+        d.tma_row = (f * p.B_total + frame) * p.H + ey.w0;
+        d.tma_k = (g >= p.F && n_items > 0) ? (ey.e1 + 7) >> 3 : 0;          // the first sweep reads no q (q = 0)
+        d.pad = 0;
+        sm.desc[g % CV_DR] = d;
+    }
+    const int last = min(count, total - first) - 1;              // last planned lane (>= 0 when anything was planned)
+    if (last >= 0) {
+        geom = __shfl_sync(0xffffffffu, my_geom, last);
+        key = __shfl_sync(0xffffffffu, my_key, last);
+    }
 }
 
-// Does step g read q through a TMA box (issued CV_PF steps earlier, awaited just before the step)?
-__device__ __forceinline__ bool step_loads_q(const Smem &sm, const CParams &p, int g, int total)
+// Control warp: table entries of steps [first, first + 16) into the ring, one 16-byte cp.async per lane.
+__device__ __forceinline__ void fetch_table(Smem &sm, const CParams &p, int first, int lane, int ci, int cj, int total)
 {
-    if (g < p.F || g >= total) return false;                         // the first sweep reads no q (q = 0)
-    return sm.tab[g % CV_TR][0].nw > 0 && sm.tab[g % CV_TR][1].nw > 0;
+    const int g = first + (lane >> 1), ax = lane & 1;
+    if (g < total) {
+        const AxisEntry *src = ax ? p.tabx + (size_t)g * p.NC + cj : p.taby + (size_t)g * p.NR + ci;
+        cp_async16((unsigned)__cvta_generic_to_shared(&sm.tab[g % CV_TR][ax]), src);
+    }
+    cp_async_commit();
 }
 
 // Arrival chunk k of the step described by (Y, X): 32 consecutive positions of one line.  Lines: the
@@ -426,7 +455,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
 
     // ---- prologue: families and the first table entries into shared memory; x <- y on the tile ----
     for (int i = tid; i < p.F; i += CV_NT) sm.fams[i] = p.fams[i];
-    for (int i = tid; i < 2 * min(total, CV_LA + 1); i += CV_NT) {
+    for (int i = tid; i < 2 * min(total, 2 * CV_BATCH); i += CV_NT) {
         const int g = i >> 1, ax = i & 1;
         sm.tab[g % CV_TR][ax] = ax ? p.tabx[(size_t)g * p.NC + cj] : p.taby[(size_t)g * p.NR + ci];
     }
@@ -440,15 +469,15 @@ conveyor_kernel(const __grid_constant__ CParams p)
             sm.xs[tidx(r, c)] = p.y[frame_off + (size_t)r * p.W + c];
         }
     }
-    ControlState cs;                            // control lane only
-    cs.geom = 0; cs.key = -1; cs.phase = 0;
     const unsigned long long frame_off_q = (unsigned long long)(p.frame0 + bl) * p.H * p.Wq;
     const unsigned long long plane = (unsigned long long)p.B_total * p.H * p.Wq;
-    if (tid == CV_NCW * 32) {
-        for (int i = 0; i < CV_NST; ++i) mbar_init(&sm.qbar[i], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        cs.plane_f = frame_off_q;
-        make_desc(sm, p, cs, 0, 0, 0, total);
+    int geom = 0, key = -1;                     // control warp: geometry id / key of the last planned step
+    if (warp == CV_NCW) {
+        if (lane == 0) {
+            for (int i = 0; i < CV_NST; ++i) mbar_init(&sm.qbar[i], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        plan_steps(sm, p, 0, CV_AHEAD, lane, total, frame_off_q, plane, p.frame0 + bl, geom, key);
     }
     __syncthreads();
 
@@ -458,8 +487,8 @@ conveyor_kernel(const __grid_constant__ CParams p)
         lc.geom = -1; lc.nwin = 0; lc.rr0 = lc.colofs = lc.lq = lc.lg = 0;
         int g = 0;
         while (g < total) {
-            const int f = sm.desc[g & 1].f;
-            const int g_end = g + sm.desc[g & 1].run_left;
+            const int f = sm.desc[g % CV_DR].f;
+            const int g_end = g + sm.desc[g % CV_DR].run_left;
             const CFamily fam = sm.fams[f];
             switch (fam.side) {
                 case 1: run_steps<1, cv_kr(1), WQ>(sm, p, lc, g, g_end, fam.c, fam.sqrt_c, warp, lane, cta, total); break;
@@ -477,42 +506,39 @@ conveyor_kernel(const __grid_constant__ CParams p)
             if (g < g_end) return;                                   // a run was cut short: abort
         }
     } else if (warp == CV_NCW) {
-        // =============== control warp: q boxes by TMA, table prefetch, next step's descriptor ============
-        int f1 = 1 % p.F;                      // family of step g + 1
-        int fp = CV_PF % p.F;                  // family of step g + CV_PF
+        // =============== control warp: plans steps in batches; per step only the TMA order and its wait ====
         int st1 = 1 % CV_NST;                  // q stage of step g + 1
         int stp = CV_PF % CV_NST;              // q stage of step g + CV_PF
-        if (lane == 0) {
-            cs.plane_f = frame_off_q + (unsigned long long)f1 * plane;
-            cs.row_fp = (fp * p.B_total + p.frame0 + bl) * p.H;
-        }
+        unsigned phase = 0;                    // bit s: parity the next wait on q stage s has to use
         for (int g = 0; g < total; ++g) {
-            if (lane == 0 && step_loads_q(sm, p, g + CV_PF, total)) {      // the q box of step g + CV_PF
-                const AxisEntry qy = sm.tab[(g + CV_PF) % CV_TR][0], qx = sm.tab[(g + CV_PF) % CV_TR][1];
-                const int k = (qy.e1 + 7) >> 3;                              // box of 8k rows, qp columns
-                mbar_expect_tx(&sm.qbar[stp], (unsigned)(k * 8 * p.qp * 4));
-                tma_load_2d(sm.qs + (size_t)stp * (CV_PW * CV_PW), &p.qmap[k - 1], qx.e0, cs.row_fp + qy.w0, &sm.qbar[stp]);  // column: 16-byte aligned
+            if ((g & (CV_BATCH - 1)) == 0) {
+                // table entries of steps [g + 32, g + 48); those fetched 16 steps ago are complete and visible
+                cp_async_wait<0>();
+                __syncwarp();
+                fetch_table(sm, p, g + 2 * CV_BATCH, lane, ci, cj, total);
+                plan_steps(sm, p, g + CV_AHEAD, CV_BATCH, lane, total, frame_off_q, plane, p.frame0 + bl, geom, key);
+                __syncwarp();
             }
-            const int gt = g + CV_LA + 1;
-            if (gt < total && lane < 2) {
-                const AxisEntry *src = lane ? p.tabx + (size_t)gt * p.NC + cj : p.taby + (size_t)gt * p.NR + ci;
-                cp_async16((unsigned)__cvta_generic_to_shared(&sm.tab[gt % CV_TR][lane]), src);
+            if (lane == 0) {
+                if (g + CV_PF < total) {                             // order the q box of step g + CV_PF
+                    const StepDesc &d = sm.desc[(g + CV_PF) % CV_DR];
+                    const int k = d.tma_k;
+                    if (k > 0) {
+                        mbar_expect_tx(&sm.qbar[stp], (unsigned)(k * 8 * p.qp * 4));
+                        tma_load_2d(sm.qs + (size_t)stp * (CV_PW * CV_PW), &p.qmap[k - 1], d.tma_col, d.tma_row, &sm.qbar[stp]);
+                    }
+                }
+                CV_STAMP(7);
+                if (g + 1 < total && sm.desc[(g + 1) % CV_DR].tma_k > 0) {   // q of step g+1 has landed
+                    const unsigned parity = (phase >> st1) & 1u;
+                    const long long t0 = clock64();
+                    while (!mbar_try_wait(&sm.qbar[st1], parity))
+                        if (clock64() - t0 > 2000000000LL) { atomicExch(p.status, 1); break; }
+                    phase ^= 1u << st1;
+                }
+                CV_STAMP(3);
             }
-            cp_async_commit();
-            if (lane == 0) CV_STAMP(7);
-            if (lane == 0 && g + 1 < total) make_desc(sm, p, cs, g + 1, f1, st1, total);
-            cp_async_wait<CV_PF - 1>();
-            if (lane == 0 && step_loads_q(sm, p, g + 1, total)) {            // q of step g+1 has landed
-                const unsigned parity = (cs.phase >> st1) & 1u;
-                const long long t0 = clock64();
-                while (!mbar_try_wait(&sm.qbar[st1], parity))
-                    if (clock64() - t0 > 2000000000LL) { atomicExch(p.status, 1); break; }
-                cs.phase ^= 1u << st1;
-            }
-            if (lane == 0) CV_STAMP(3);
             CV_STEP_BARRIER();
-            if (++f1 == p.F) { f1 = 0; cs.plane_f = frame_off_q; } else cs.plane_f += plane;
-            if (++fp == p.F) { fp = 0; cs.row_fp = (p.frame0 + bl) * p.H; } else cs.row_fp += p.B_total * p.H;
             if (++st1 == CV_NST) st1 = 0;
             if (++stp == CV_NST) stp = 0;
         }
