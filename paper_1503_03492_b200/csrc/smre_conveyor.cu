@@ -331,7 +331,6 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
                                    c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, CV_NCW * 32, warp, lane);
         }
         if (warp == 0 && lane == 0) CV_STAMP(1);
-        if (warp == 8 && lane == 0) CV_STAMP(2);
         CV_STEP_BARRIER();
         if (warp == 0 && lane == 0) CV_STAMP(0);
     }
@@ -557,14 +556,14 @@ conveyor_kernel(const __grid_constant__ CParams p)
         int prog_iter = -1;                     // step at which prog_pend was requested (-1: none in flight)
         for (int g = 0; g < total; ++g) {
             if (g > 0) {
-                if (lane >= 1 && lane <= 3) {                        // the ring slot must have been read
-                    // the neighbour's counter is re-read only when the ring is half used, and the value is
-                    // picked up a few steps later: the load must never sit on this warp's critical path
-                    if (prog_iter >= 0 && g >= prog_iter + 3) { prog_seen = max(prog_seen, prog_pend); prog_iter = -1; }
-                    if ((int)prog_seen + CV_D < g) {
-                        prog_seen = poll_prog(my_nbr_prog, (unsigned)(g - CV_D), p.status);
-                        prog_iter = -1;
-                    } else if (prog_iter < 0 && (int)prog_seen + CV_D / 2 < g) {
+                if ((g & 3) == 1 && lane >= 1 && lane <= 3) {
+                    // Ring slots g .. g+3 must have been read by the receiver: its counter must have reached
+                    // g + 3 - CV_D.  The counter is re-read only when the ring is half used, and the value is
+                    // picked up 4 steps later: the load never sits on this warp's critical path.
+                    if (prog_iter >= 0) { prog_seen = max(prog_seen, prog_pend); prog_iter = -1; }
+                    if ((int)prog_seen + CV_D < g + 3) {
+                        prog_seen = poll_prog(my_nbr_prog, (unsigned)(g + 3 - CV_D), p.status);
+                    } else if ((int)prog_seen + CV_D / 2 < g + 3) {
                         prog_pend = ld_u32_gpu(my_nbr_prog);
                         prog_iter = g;
                     }
@@ -573,61 +572,99 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
                 const int slot = (g % CV_D) * CV_MBW;
                 const unsigned long long tag = (unsigned long long)(unsigned)g << 32;
-                for (int c = px.L; c < px.D; ++c)                    // column strip: columns [L, D), all rows
-                    for (int r = py.L + lane; r < py.R; r += 32) {
-                        unsigned long long *box = (r < py.D) ? box_ul : box_l;
-                        st_u64_gpu(box + slot + mbox_col_word(r, c), tag | __float_as_uint(sm.xs[tidx(r, c)]));
+                // departing lines: the columns [L, D) (all rows), then the rows [L, D) x columns [D, R);
+                // two 32-lane chunks per line, two chunks per round (the usual step has exactly one column)
+                const int ncl = px.D - px.L;
+                const int nchunks = (py.R > py.L && px.R > px.L) ? 2 * (ncl + (px.R > px.D ? py.D - py.L : 0)) : 0;
+                for (int k0 = 0; k0 < nchunks; k0 += 2) {
+                    unsigned long long *dst[2];
+                    float val[2];
+                    bool ok[2];
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const int line = (k0 >> 1), pos = (u << 5) + lane;
+                        int r, c, word;
+                        unsigned long long *box;
+                        if (line < ncl) {
+                            c = px.L + line; r = py.L + pos;
+                            ok[u] = r < py.R;
+                            word = mbox_col_word(r, c);
+                            box = (r < py.D) ? box_ul : box_l;
+                        } else {
+                            r = py.L + (line - ncl); c = px.D + pos;
+                            ok[u] = c < px.R;
+                            word = mbox_row_word(r, c);
+                            box = box_u;
+                        }
+                        dst[u] = box + slot + word;
+                        val[u] = ok[u] ? sm.xs[tidx(r, c)] : 0.0f;
                     }
-                for (int r = py.L; r < py.D; ++r)                    // row strip: rows [L, D), columns [D, R)
-                    for (int c = px.D + lane; c < px.R; c += 32)
-                        st_u64_gpu(box_u + slot + mbox_row_word(r, c), tag | __float_as_uint(sm.xs[tidx(r, c)]));
+#pragma unroll
+                    for (int u = 0; u < 2; ++u)
+                        if (ok[u]) st_u64_gpu(dst[u], tag | __float_as_uint(val[u]));
+                }
             }
             if (lane == 0) CV_STAMP(4);
             CV_STEP_BARRIER();
         }
     } else {
         // =============== receiver warp: arrivals of step g+1 into the tile ================================
+        // The first line (two chunks) of every step -- all there is in the usual step -- is located and
+        // requested one step ahead; its geometry is kept in registers for the deposit a step later.
         unsigned long long *const my_box = p.mbox + (size_t)cta * CV_D * CV_MBW;
-        unsigned long long pend[4] = {0, 0, 0, 0};   // the first four chunks of step g+2, loaded a step ahead
+        unsigned long long pend[2] = {0, 0};
+        int pxi[2] = {0, 0}, pwd[2] = {0, 0}, pn = 0;
+        bool pok[2] = {false, false};
         int status_pend = 0;                         // lane 0: the failure flag, loaded a step ahead
+        auto locate = [&](int step) {                // chunks 0, 1 of `step`; requests their mailbox words
+            const AxisEntry my = sm.tab[step % CV_TR][0], mx = sm.tab[step % CV_TR][1];
+            const unsigned long long *box2 = my_box + (size_t)(step % CV_D) * CV_MBW;
+            pn = arrival_chunks(my, mx);
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                int r, c;
+                pok[u] = u < pn && arrival_chunk(my, mx, u, lane, r, c, pwd[u]);
+                pxi[u] = tidx(r, c);
+                pend[u] = ld_u64_gpu(box2 + (pok[u] ? pwd[u] : 0));      // unconditional: nothing waits on it
+            }
+        };
+        if (total > 1) locate(1);
         for (int g = 0; g < total; ++g) {
             if (g + 1 < total) {
-                const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
                 const unsigned long long *box = my_box + (size_t)((g + 1) % CV_D) * CV_MBW;
                 const unsigned tag = (unsigned)(g + 1);
-                const int nchunks = arrival_chunks(ny, nx);
-                for (int k0 = 0; k0 < nchunks; k0 += 4) {
-                    unsigned long long w[4];
-                    int xi[4], wd[4];
-                    bool ok[4];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        int r, c;
-                        ok[u] = (k0 + u < nchunks) && arrival_chunk(ny, nx, k0 + u, lane, r, c, wd[u]);
-                        xi[u] = tidx(r, c);
-                        w[u] = (k0 == 0) ? pend[u] : (ok[u] ? ld_u64_gpu(box + wd[u]) : 0ull);
+                for (int u = 0; u < 2; ++u)
+                    if (pok[u]) {
+                        unsigned long long w = pend[u];
+                        if ((unsigned)(w >> 32) != tag) w = poll_tag(box + pwd[u], tag, p.status);
+                        sm.xs[pxi[u]] = __uint_as_float((unsigned)w);
                     }
+                if (pn > 2) {                                        // rare: several lines arrive
+                    const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
+                    for (int k0 = 2; k0 < pn; k0 += 4) {
+                        unsigned long long w[4];
+                        int xi[4], wd[4];
+                        bool ok[4];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u)
-                        if (ok[u]) {
-                            if ((unsigned)(w[u] >> 32) != tag) w[u] = poll_tag(box + wd[u], tag, p.status);
-                            sm.xs[xi[u]] = __uint_as_float((unsigned)w[u]);
+                        for (int u = 0; u < 4; ++u) {
+                            int r, c;
+                            ok[u] = (k0 + u < pn) && arrival_chunk(ny, nx, k0 + u, lane, r, c, wd[u]);
+                            xi[u] = tidx(r, c);
+                            w[u] = ok[u] ? ld_u64_gpu(box + wd[u]) : 0ull;
                         }
+#pragma unroll
+                        for (int u = 0; u < 4; ++u)
+                            if (ok[u]) {
+                                if ((unsigned)(w[u] >> 32) != tag) w[u] = poll_tag(box + wd[u], tag, p.status);
+                                sm.xs[xi[u]] = __uint_as_float((unsigned)w[u]);
+                            }
+                    }
                 }
                 __syncwarp();
+                if (lane == 0) CV_STAMP(2);
                 if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // step g+1 has been read
-#pragma unroll
-                for (int u = 0; u < 4; ++u) pend[u] = 0;
-                if (g + 2 < total) {
-                    const AxisEntry my = sm.tab[(g + 2) % CV_TR][0], mx = sm.tab[(g + 2) % CV_TR][1];
-                    const unsigned long long *box2 = my_box + (size_t)((g + 2) % CV_D) * CV_MBW;
-                    const int mchunks = arrival_chunks(my, mx);
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        int r, c, wd;
-                        if (u < mchunks && arrival_chunk(my, mx, u, lane, r, c, wd)) pend[u] = ld_u64_gpu(box2 + wd);
-                    }
-                }
+                if (g + 2 < total) locate(g + 2);
             }
             if (lane == 0 && (g & 7) == 3) {
                 if (status_pend) sm.abort = 1;
