@@ -4,10 +4,10 @@
 A "step" = one smre_project call = the whole hot path over one
 synthetic workload.  Default workload = BASELINE.json configs[1]: 512x512, sides 1-8 (204
 families), standard Dykstra, 200 sweeps.  Metric: Dykstra sweeps/s (window-projections/s is
-reported beside it).  N > 1: replicas only (DESIGN.md sec. 9) -- every rank projects its own
+reported beside it).  N > 1: replicas only (DESIGN.md sec. 10) -- every rank projects its own
 image, no collective on the data path; value = sweeps of all ranks / max-over-ranks time.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--schedule auto|graph|persistent]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--schedule auto|graph|conveyor]
   python bench.py --impl reference ...      # times the fp64 CPU oracle (rank 0 only)
 """
 from __future__ import annotations
@@ -149,7 +149,7 @@ def run_gpu(args, w, rank, world):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     sched = {"auto": smre.SMRE_SCHED_AUTO, "graph": smre.SMRE_SCHED_GRAPH,
-             "persistent": smre.SMRE_SCHED_PERSISTENT}[args.schedule]
+             "persistent": smre.SMRE_SCHED_PERSISTENT, "conveyor": smre.SMRE_SCHED_PERSISTENT}[args.schedule]
     nums = workload_numbers(w)
     sol = smre.Solver(w.H, w.W, w.sides, w.c, w.variant, w.batch, sched)
     stream = torch.cuda.Stream()
@@ -206,12 +206,10 @@ def run_gpu(args, w, rank, world):
     launch = sol.last_launch
     wall_e, dev_e, _ = timed(step_host, max(1, args.warmup // 2), args.steps, False)
 
+    from paper_1503_03492_b200.replicas import max_over_ranks as _max_over_ranks
+
     def max_over_ranks(v):
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return _max_over_ranks(v, dist, "cuda")
 
     dev, dev_e, wall_e = max_over_ranks(dev), max_over_ranks(dev_e), max_over_ranks(wall_e)
     sweeps_total = w.n_sweeps * args.steps * world
@@ -221,7 +219,7 @@ def run_gpu(args, w, rank, world):
     if rank == 0:
         peak, peak_src, _ = measured_peaks()
         per_launch_s = dev / args.steps                       # persistent: one kernel = one step
-        kernel = "persistent_sweep_kernel" if launch[0] == smre.SMRE_SCHED_PERSISTENT else "family_pass_kernel"
+        kernel = "conveyor_kernel" if launch[0] == smre.SMRE_SCHED_PERSISTENT else "family_pass_kernel"
         if w.variant != "standard":
             kernel = "icd_shift_kernel"
         achieved = nums["bytes_per_step"] / per_launch_s / 1e9
@@ -246,7 +244,7 @@ def run_gpu(args, w, rank, world):
             "config": {"workload": w.name, "note": w.note, "variant": w.variant, "n_sweeps": w.n_sweeps,
                        "H": w.H, "W": w.W, "batch": w.batch, "families": nums["families"],
                        "windows_per_sweep": nums["windows_per_sweep"],
-                       "schedule": {1: "graph", 2: "persistent"}.get(launch[0], str(launch[0])),
+                       "schedule": {1: "graph", 2: "conveyor"}.get(launch[0], str(launch[0])),
                        "tiles": [launch[2], launch[3]],
                        "l2": "q planes (>L2) re-zeroed every step" if flush is None else "256 MiB flush between steps",
                        "parallelism": "replicas only" if world > 1 else "1 GPU"},
@@ -272,7 +270,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1)")
     ap.add_argument("--n-sweeps", type=int, default=None, help="override the config's sweep count (debug)")
-    ap.add_argument("--schedule", default="auto", choices=["auto", "graph", "persistent"])
+    ap.add_argument("--schedule", default="auto", choices=["auto", "graph", "persistent", "conveyor"])
     ap.add_argument("--ref-sweeps", type=int, default=50, help="oracle sample size in sweeps (~15 s on C1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -55,6 +55,21 @@ def test_schedulers_agree_bitwise(idx, n):
         assert np.array_equal(x, res["graph"]), name
 
 
+# ---- the conveyor is deterministic: repeated calls give the graph scheduler's bits every time ---------------
+def test_conveyor_repeatable():
+    for idx, n, reps in ((0, 20, 25), (1, 2, 6)):
+        w = si.config(idx)
+        ref, _ = gpu_project(w.y, w.sides, w.c, "standard", n, smre.SMRE_SCHED_GRAPH)
+        sol = smre.Solver(w.H, w.W, w.sides, w.c, "standard", 1, smre.SMRE_SCHED_PERSISTENT)
+        yt = torch.from_numpy(w.y).cuda()
+        for _ in range(reps):
+            x = sol.project(yt, n)
+            torch.cuda.synchronize()
+            assert sol.last_launch[0] == smre.SMRE_SCHED_PERSISTENT
+            assert np.array_equal(x.cpu().numpy(), ref)
+        sol.close()
+
+
 # ---- small, ragged, degenerate --------------------------------------------------------------------
 CASES = [
     # H, W, batch, sides, variant, sweeps
