@@ -139,7 +139,7 @@ static_assert(CV_PW == 64, "tidx assumes a 64 x 64 torus");
 __device__ __forceinline__ int mbox_col_word(int r, int c) { return ((c & (CV_SD - 1)) << 6) | (r & 63); }
 __device__ __forceinline__ int mbox_row_word(int r, int c) { return CV_SD * 64 + (((r & (CV_SD - 1)) << 6) | (c & 63)); }
 
-// Per-step descriptor (48 bytes; the compute warps read the first 32), written one step ahead by the control
+// Per-step descriptor (64 bytes; the compute warps read the first 32), written one step ahead by the control
 // warp so that the compute warps do almost no index arithmetic of their own.
 struct StepDesc {
     // v0
@@ -155,9 +155,14 @@ struct StepDesc {
     // v2: the TMA box that brings this step's q (issued CV_PF steps before the step, awaited just before it)
     int tma_col, tma_row;         // tensor coordinates: 4-aligned column, row of (family, frame, first window row)
     int tma_k;                    // box height / 8 (1..8); 0: this step reads no q
-    int pad;
+    unsigned send_x;              // sender: pixels of the first departing line that go to the up-left CTA | all-up flag << 8
+    // v3: first line (two 32-lane chunks) of the hand-off, for lane position pos: v = (var0 + pos) & 63,
+    //     mailbox word = wbase | v, tile index = xbase | v << sh.   a = wbase | xbase << 16,
+    //     b = var0 | len << 8 | sh << 16 | chunks of the whole step << 24
+    unsigned recv_a, recv_b;      // arrivals OF this step
+    unsigned send_a, send_b;      // departures AFTER this step
 };
-static_assert(sizeof(StepDesc) == 48, "StepDesc must be 48 bytes");
+static_assert(sizeof(StepDesc) == 64, "StepDesc must be 64 bytes");
 
 struct GeomDesc { int nwx, nwy, n_items, pad; };   // read by the lanes only when StepDesc::geom changes
 
@@ -394,7 +399,27 @@ __device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first
         d.tma_col = ex.e0;
         d.tma_row = (f * p.B_total + frame) * p.H + ey.w0;
         d.tma_k = (g >= p.F && n_items > 0) ? (ey.e1 + 7) >> 3 : 0;          // the first sweep reads no q (q = 0)
-        d.pad = 0;
+        {   // first arriving line: the first column of the column strip, else the first row of the row strip
+            const int h = ey.R - ey.L, live = (h > 0 && ex.R > ex.L);
+            const int ncl = ex.R - ex.A, nrl = (ex.A > ex.L) ? ey.R - ey.A : 0;
+            const int chunks = live ? 2 * (ncl + nrl) : 0;
+            unsigned wbase = 0, xbase = 0, var0 = 0, len = 0, sh = 0;
+            if (live && ncl > 0) { wbase = (ex.A & (CV_SD - 1)) << 6; xbase = ex.A & 63; var0 = ey.L & 63; len = h; sh = 6; }
+            else if (live && nrl > 0) { wbase = CV_SD * 64 + ((ey.A & (CV_SD - 1)) << 6); xbase = (ey.A & 63) << 6; var0 = ex.L & 63; len = ex.A - ex.L; sh = 0; }
+            d.recv_a = wbase | (xbase << 16);
+            d.recv_b = var0 | (len << 8) | (sh << 16) | ((unsigned)chunks << 24);
+        }
+        {   // first departing line: the first column of [L, D), else the first row of [L, D) x [D, R)
+            const int h = ey.R - ey.L, live = (h > 0 && ex.R > ex.L);
+            const int ncl = ex.D - ex.L, nrl = (ex.R > ex.D) ? ey.D - ey.L : 0;
+            const int chunks = live ? 2 * (ncl + nrl) : 0;
+            unsigned wbase = 0, xbase = 0, var0 = 0, len = 0, sh = 0, nul = 0, up = 0;
+            if (live && ncl > 0) { wbase = (ex.L & (CV_SD - 1)) << 6; xbase = ex.L & 63; var0 = ey.L & 63; len = h; sh = 6; nul = ey.D - ey.L; }
+            else if (live && nrl > 0) { wbase = CV_SD * 64 + ((ey.L & (CV_SD - 1)) << 6); xbase = (ey.L & 63) << 6; var0 = ex.D & 63; len = ex.R - ex.D; sh = 0; up = 1; }
+            d.send_a = wbase | (xbase << 16);
+            d.send_b = var0 | (len << 8) | (sh << 16) | ((unsigned)chunks << 24);
+            d.send_x = nul | (up << 8);
+        }
         sm.desc[g % CV_DR] = d;
     }
     const int last = min(count, total - first) - 1;              // last planned lane (>= 0 when anything was planned)
@@ -569,39 +594,62 @@ conveyor_kernel(const __grid_constant__ CParams p)
                     }
                 }
                 __syncwarp();
-                const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
                 const int slot = (g % CV_D) * CV_MBW;
                 const unsigned long long tag = (unsigned long long)(unsigned)g << 32;
-                // departing lines: the columns [L, D) (all rows), then the rows [L, D) x columns [D, R);
-                // two 32-lane chunks per line, two chunks per round (the usual step has exactly one column)
-                const int ncl = px.D - px.L;
-                const int nchunks = (py.R > py.L && px.R > px.L) ? 2 * (ncl + (px.R > px.D ? py.D - py.L : 0)) : 0;
-                for (int k0 = 0; k0 < nchunks; k0 += 2) {
-                    unsigned long long *dst[2];
+                // first departing line of step g-1 (all there is in the usual step), from the planner
+                const uint4 ln = *reinterpret_cast<const uint4 *>(&sm.desc[(g - 1) % CV_DR].recv_a);   // {recv_a, recv_b, send_a, send_b}
+                const unsigned sx = sm.desc[(g - 1) % CV_DR].send_x;
+                const int nchunks = (int)(ln.w >> 24);
+                if (nchunks > 0) {
+                    const unsigned var0 = ln.w & 63u, len = (ln.w >> 8) & 0xffu, sh = (ln.w >> 16) & 0xffu;
+                    const unsigned wbase = ln.z & 0xffffu, xbase = ln.z >> 16;
+                    const unsigned nul = sx & 0xffu;
+                    unsigned long long *const box_lo = (sx >> 8) ? box_u : box_l;      // row line: everything goes up
                     float val[2];
-                    bool ok[2];
+                    unsigned wd[2];
 #pragma unroll
                     for (int u = 0; u < 2; ++u) {
-                        const int line = (k0 >> 1), pos = (u << 5) + lane;
-                        int r, c, word;
-                        unsigned long long *box;
-                        if (line < ncl) {
-                            c = px.L + line; r = py.L + pos;
-                            ok[u] = r < py.R;
-                            word = mbox_col_word(r, c);
-                            box = (r < py.D) ? box_ul : box_l;
-                        } else {
-                            r = py.L + (line - ncl); c = px.D + pos;
-                            ok[u] = c < px.R;
-                            word = mbox_row_word(r, c);
-                            box = box_u;
-                        }
-                        dst[u] = box + slot + word;
-                        val[u] = ok[u] ? sm.xs[tidx(r, c)] : 0.0f;
+                        const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
+                        wd[u] = wbase | v;
+                        val[u] = pos < len ? sm.xs[xbase | (v << sh)] : 0.0f;
                     }
 #pragma unroll
-                    for (int u = 0; u < 2; ++u)
-                        if (ok[u]) st_u64_gpu(dst[u], tag | __float_as_uint(val[u]));
+                    for (int u = 0; u < 2; ++u) {
+                        const unsigned pos = (u << 5) + lane;
+                        if (pos < len)
+                            st_u64_gpu((pos < nul ? box_ul : box_lo) + slot + wd[u], tag | __float_as_uint(val[u]));
+                    }
+                }
+                if (nchunks > 2) {                                   // rare: several lines depart
+                    const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
+                    const int ncl = px.D - px.L;
+                    for (int k0 = 2; k0 < nchunks; k0 += 2) {
+                        unsigned long long *dst[2];
+                        float val[2];
+                        bool ok[2];
+#pragma unroll
+                        for (int u = 0; u < 2; ++u) {
+                            const int line = (k0 >> 1), pos = (u << 5) + lane;
+                            int r, c, word;
+                            unsigned long long *box;
+                            if (line < ncl) {
+                                c = px.L + line; r = py.L + pos;
+                                ok[u] = r < py.R;
+                                word = mbox_col_word(r, c);
+                                box = (r < py.D) ? box_ul : box_l;
+                            } else {
+                                r = py.L + (line - ncl); c = px.D + pos;
+                                ok[u] = c < px.R;
+                                word = mbox_row_word(r, c);
+                                box = box_u;
+                            }
+                            dst[u] = box + slot + word;
+                            val[u] = ok[u] ? sm.xs[tidx(r, c)] : 0.0f;
+                        }
+#pragma unroll
+                        for (int u = 0; u < 2; ++u)
+                            if (ok[u]) st_u64_gpu(dst[u], tag | __float_as_uint(val[u]));
+                    }
                 }
             }
             if (lane == 0) CV_STAMP(4);
@@ -616,16 +664,19 @@ conveyor_kernel(const __grid_constant__ CParams p)
         int pxi[2] = {0, 0}, pwd[2] = {0, 0}, pn = 0;
         bool pok[2] = {false, false};
         int status_pend = 0;                         // lane 0: the failure flag, loaded a step ahead
-        auto locate = [&](int step) {                // chunks 0, 1 of `step`; requests their mailbox words
-            const AxisEntry my = sm.tab[step % CV_TR][0], mx = sm.tab[step % CV_TR][1];
+        auto locate = [&](int step) {                // chunks 0, 1 of `step` from the planner; requests their words
+            const uint2 ln = *reinterpret_cast<const uint2 *>(&sm.desc[step % CV_DR].recv_a);
             const unsigned long long *box2 = my_box + (size_t)(step % CV_D) * CV_MBW;
-            pn = arrival_chunks(my, mx);
+            pn = (int)(ln.y >> 24);
+            const unsigned var0 = ln.y & 63u, len = (ln.y >> 8) & 0xffu, sh = (ln.y >> 16) & 0xffu;
+            const unsigned wbase = ln.x & 0xffffu, xbase = ln.x >> 16;
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-                int r, c;
-                pok[u] = u < pn && arrival_chunk(my, mx, u, lane, r, c, pwd[u]);
-                pxi[u] = tidx(r, c);
-                pend[u] = ld_u64_gpu(box2 + (pok[u] ? pwd[u] : 0));      // unconditional: nothing waits on it
+                const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
+                pok[u] = pos < len;
+                pwd[u] = (int)(wbase | v);
+                pxi[u] = (int)(xbase | (v << sh));
+                pend[u] = ld_u64_gpu(box2 + pwd[u]);                     // unconditional: nothing waits on it
             }
         };
         if (total > 1) locate(1);
