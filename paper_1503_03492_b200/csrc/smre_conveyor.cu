@@ -139,7 +139,7 @@ static_assert(CV_PW == 64, "tidx assumes a 64 x 64 torus");
 __device__ __forceinline__ int mbox_col_word(int r, int c) { return ((c & (CV_SD - 1)) << 6) | (r & 63); }
 __device__ __forceinline__ int mbox_row_word(int r, int c) { return CV_SD * 64 + (((r & (CV_SD - 1)) << 6) | (c & 63)); }
 
-// Per-step descriptor (64 bytes; the compute warps read the first 32), written one step ahead by the control
+// Per-step descriptor (80 bytes; the compute warps read the first 32), written one step ahead by the control
 // warp so that the compute warps do almost no index arithmetic of their own.
 struct StepDesc {
     // v0
@@ -155,14 +155,15 @@ struct StepDesc {
     // v2: the TMA box that brings this step's q (issued CV_PF steps before the step, awaited just before it)
     int tma_col, tma_row;         // tensor coordinates: 4-aligned column, row of (family, frame, first window row)
     int tma_k;                    // box height / 8 (1..8); 0: this step reads no q
-    unsigned send_x;              // sender: pixels of the first departing line that go to the up-left CTA | all-up flag << 8
-    // v3: first line (two 32-lane chunks) of the hand-off, for lane position pos: v = (var0 + pos) & 63,
-    //     mailbox word = wbase | v, tile index = xbase | v << sh.   a = wbase | xbase << 16,
-    //     b = var0 | len << 8 | sh << 16 | chunks of the whole step << 24
-    unsigned recv_a, recv_b;      // arrivals OF this step
-    unsigned send_a, send_b;      // departures AFTER this step
+    unsigned send_x;              // sender, per line (A: bits 0-15, B: bits 16-31): pixels that go to the up-left CTA | all-up flag << 8
+    // v3, v4: the first two lines (two 32-lane chunks each) of the hand-off, enough for every step except the
+    //     changes of window edge.  For lane position pos: v = (var0 + pos) & 63, mailbox word = wbase | v,
+    //     tile index = xbase | v << sh.   a = wbase | xbase << 16,  b = var0 | len << 8 | sh << 16 | chunks of
+    //     the whole step << 24 (line A only)
+    unsigned recv_a[2], recv_b[2];   // arrivals OF this step          (stored a0, a1, b0, b1)
+    unsigned send_a[2], send_b[2];   // departures AFTER this step
 };
-static_assert(sizeof(StepDesc) == 64, "StepDesc must be 64 bytes");
+static_assert(sizeof(StepDesc) == 80, "StepDesc must be 80 bytes");
 
 struct GeomDesc { int nwx, nwy, n_items, pad; };   // read by the lanes only when StepDesc::geom changes
 
@@ -399,26 +400,37 @@ __device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first
         d.tma_col = ex.e0;
         d.tma_row = (f * p.B_total + frame) * p.H + ey.w0;
         d.tma_k = (g >= p.F && n_items > 0) ? (ey.e1 + 7) >> 3 : 0;          // the first sweep reads no q (q = 0)
-        {   // first arriving line: the first column of the column strip, else the first row of the row strip
+        {
+            // Lines of a hand-off in order: the columns of the column strip (all tile rows), then the rows of
+            // the row strip.  line(k) describes line k (k = 0, 1) of the arrivals (arr) or departures of this step.
             const int h = ey.R - ey.L, live = (h > 0 && ex.R > ex.L);
-            const int ncl = ex.R - ex.A, nrl = (ex.A > ex.L) ? ey.R - ey.A : 0;
-            const int chunks = live ? 2 * (ncl + nrl) : 0;
-            unsigned wbase = 0, xbase = 0, var0 = 0, len = 0, sh = 0;
-            if (live && ncl > 0) { wbase = (ex.A & (CV_SD - 1)) << 6; xbase = ex.A & 63; var0 = ey.L & 63; len = h; sh = 6; }
-            else if (live && nrl > 0) { wbase = CV_SD * 64 + ((ey.A & (CV_SD - 1)) << 6); xbase = (ey.A & 63) << 6; var0 = ex.L & 63; len = ex.A - ex.L; sh = 0; }
-            d.recv_a = wbase | (xbase << 16);
-            d.recv_b = var0 | (len << 8) | (sh << 16) | ((unsigned)chunks << 24);
-        }
-        {   // first departing line: the first column of [L, D), else the first row of [L, D) x [D, R)
-            const int h = ey.R - ey.L, live = (h > 0 && ex.R > ex.L);
-            const int ncl = ex.D - ex.L, nrl = (ex.R > ex.D) ? ey.D - ey.L : 0;
-            const int chunks = live ? 2 * (ncl + nrl) : 0;
-            unsigned wbase = 0, xbase = 0, var0 = 0, len = 0, sh = 0, nul = 0, up = 0;
-            if (live && ncl > 0) { wbase = (ex.L & (CV_SD - 1)) << 6; xbase = ex.L & 63; var0 = ey.L & 63; len = h; sh = 6; nul = ey.D - ey.L; }
-            else if (live && nrl > 0) { wbase = CV_SD * 64 + ((ey.L & (CV_SD - 1)) << 6); xbase = (ey.L & 63) << 6; var0 = ex.D & 63; len = ex.R - ex.D; sh = 0; up = 1; }
-            d.send_a = wbase | (xbase << 16);
-            d.send_b = var0 | (len << 8) | (sh << 16) | ((unsigned)chunks << 24);
-            d.send_x = nul | (up << 8);
+            auto line = [&](bool arr, int k, unsigned &a, unsigned &b, unsigned &x) {
+                const int c_lo = arr ? ex.A : ex.L, c_hi = arr ? ex.R : ex.D;          // column strip [c_lo, c_hi)
+                const int r_lo = arr ? ey.A : ey.L, r_hi = arr ? ey.R : ey.D;          // row strip rows [r_lo, r_hi)
+                const int rc_lo = arr ? ex.L : ex.D, rc_hi = arr ? ex.A : ex.R;        // ... and its columns
+                const int ncl = c_hi - c_lo, nrl = (rc_hi > rc_lo) ? r_hi - r_lo : 0;
+                const int chunks = live ? 2 * (ncl + nrl) : 0;
+                unsigned wbase = 0, xbase = 0, var0 = 0, len = 0, sh = 0;
+                x = 0;
+                if (live && k < ncl) {
+                    const int c = c_lo + k;
+                    wbase = (c & (CV_SD - 1)) << 6; xbase = c & 63; var0 = ey.L & 63; len = h; sh = 6;
+                    x = arr ? 0u : (unsigned)(ey.D - ey.L);                             // these go up-left
+                } else if (live && k < ncl + nrl) {
+                    const int r = r_lo + (k - ncl);
+                    wbase = CV_SD * 64 + ((r & (CV_SD - 1)) << 6); xbase = (r & 63) << 6; var0 = rc_lo & 63;
+                    len = rc_hi - rc_lo; sh = 0;
+                    x = 1u << 8;                                                        // everything goes up
+                }
+                a = wbase | (xbase << 16);
+                b = var0 | (len << 8) | (sh << 16) | (k == 0 ? (unsigned)chunks << 24 : 0u);
+            };
+            unsigned x0, x1;
+            line(true, 0, d.recv_a[0], d.recv_b[0], x0);
+            line(true, 1, d.recv_a[1], d.recv_b[1], x1);
+            line(false, 0, d.send_a[0], d.send_b[0], x0);
+            line(false, 1, d.send_a[1], d.send_b[1], x1);
+            d.send_x = x0 | (x1 << 16);
         }
         sm.desc[g % CV_DR] = d;
     }
@@ -596,34 +608,43 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 __syncwarp();
                 const int slot = (g % CV_D) * CV_MBW;
                 const unsigned long long tag = (unsigned long long)(unsigned)g << 32;
-                // first departing line of step g-1 (all there is in the usual step), from the planner
-                const uint4 ln = *reinterpret_cast<const uint4 *>(&sm.desc[(g - 1) % CV_DR].recv_a);   // {recv_a, recv_b, send_a, send_b}
+                // the first two departing lines of step g-1 (all there is except at changes of window edge)
+                const uint4 ln = *reinterpret_cast<const uint4 *>(&sm.desc[(g - 1) % CV_DR].send_a[0]);   // {a0, a1, b0, b1}
                 const unsigned sx = sm.desc[(g - 1) % CV_DR].send_x;
-                const int nchunks = (int)(ln.w >> 24);
+                const int nchunks = (int)(ln.z >> 24);
                 if (nchunks > 0) {
-                    const unsigned var0 = ln.w & 63u, len = (ln.w >> 8) & 0xffu, sh = (ln.w >> 16) & 0xffu;
-                    const unsigned wbase = ln.z & 0xffffu, xbase = ln.z >> 16;
-                    const unsigned nul = sx & 0xffu;
-                    unsigned long long *const box_lo = (sx >> 8) ? box_u : box_l;      // row line: everything goes up
-                    float val[2];
-                    unsigned wd[2];
+                    float val[4];
+                    unsigned wd[4];
+                    bool ok[4];
 #pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
-                        wd[u] = wbase | v;
-                        val[u] = pos < len ? sm.xs[xbase | (v << sh)] : 0.0f;
+                    for (int l = 0; l < 2; ++l) {
+                        const unsigned a = l ? ln.y : ln.x, b = l ? ln.w : ln.z;
+                        const unsigned var0 = b & 63u, len = (b >> 8) & 0xffu, sh = (b >> 16) & 0xffu;
+#pragma unroll
+                        for (int u = 0; u < 2; ++u) {
+                            const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
+                            ok[2 * l + u] = pos < len;
+                            wd[2 * l + u] = (a & 0xffffu) | v;
+                            val[2 * l + u] = pos < len ? sm.xs[(a >> 16) | (v << sh)] : 0.0f;
+                        }
                     }
 #pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const unsigned pos = (u << 5) + lane;
-                        if (pos < len)
-                            st_u64_gpu((pos < nul ? box_ul : box_lo) + slot + wd[u], tag | __float_as_uint(val[u]));
+                    for (int l = 0; l < 2; ++l) {
+                        const unsigned x = l ? sx >> 16 : sx & 0xffffu;
+                        unsigned long long *const box_lo = (x >> 8) ? box_u : box_l;    // row line: everything goes up
+#pragma unroll
+                        for (int u = 0; u < 2; ++u) {
+                            const unsigned pos = (u << 5) + lane;
+                            if (ok[2 * l + u])
+                                st_u64_gpu((pos < (x & 0xffu) ? box_ul : box_lo) + slot + wd[2 * l + u],
+                                           tag | __float_as_uint(val[2 * l + u]));
+                        }
                     }
                 }
-                if (nchunks > 2) {                                   // rare: several lines depart
+                if (nchunks > 4) {                                   // rare: more than two lines depart
                     const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
                     const int ncl = px.D - px.L;
-                    for (int k0 = 2; k0 < nchunks; k0 += 2) {
+                    for (int k0 = 4; k0 < nchunks; k0 += 2) {
                         unsigned long long *dst[2];
                         float val[2];
                         bool ok[2];
@@ -660,23 +681,26 @@ conveyor_kernel(const __grid_constant__ CParams p)
         // The first line (two chunks) of every step -- all there is in the usual step -- is located and
         // requested one step ahead; its geometry is kept in registers for the deposit a step later.
         unsigned long long *const my_box = p.mbox + (size_t)cta * CV_D * CV_MBW;
-        unsigned long long pend[2] = {0, 0};
-        int pxi[2] = {0, 0}, pwd[2] = {0, 0}, pn = 0;
-        bool pok[2] = {false, false};
+        unsigned long long pend[4] = {0, 0, 0, 0};
+        int pxi[4] = {0, 0, 0, 0}, pwd[4] = {0, 0, 0, 0}, pn = 0;
+        bool pok[4] = {false, false, false, false};
         int status_pend = 0;                         // lane 0: the failure flag, loaded a step ahead
-        auto locate = [&](int step) {                // chunks 0, 1 of `step` from the planner; requests their words
-            const uint2 ln = *reinterpret_cast<const uint2 *>(&sm.desc[step % CV_DR].recv_a);
+        auto locate = [&](int step) {                // chunks 0..3 of `step` from the planner; requests their words
+            const uint4 ln = *reinterpret_cast<const uint4 *>(&sm.desc[step % CV_DR].recv_a[0]);   // {a0, a1, b0, b1}
             const unsigned long long *box2 = my_box + (size_t)(step % CV_D) * CV_MBW;
-            pn = (int)(ln.y >> 24);
-            const unsigned var0 = ln.y & 63u, len = (ln.y >> 8) & 0xffu, sh = (ln.y >> 16) & 0xffu;
-            const unsigned wbase = ln.x & 0xffffu, xbase = ln.x >> 16;
+            pn = (int)(ln.z >> 24);
 #pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
-                pok[u] = pos < len;
-                pwd[u] = (int)(wbase | v);
-                pxi[u] = (int)(xbase | (v << sh));
-                pend[u] = ld_u64_gpu(box2 + pwd[u]);                     // unconditional: nothing waits on it
+            for (int l = 0; l < 2; ++l) {
+                const unsigned a = l ? ln.y : ln.x, b = l ? ln.w : ln.z;
+                const unsigned var0 = b & 63u, len = (b >> 8) & 0xffu, sh = (b >> 16) & 0xffu;
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
+                    pok[2 * l + u] = pos < len;
+                    pwd[2 * l + u] = (int)((a & 0xffffu) | v);
+                    pxi[2 * l + u] = (int)((a >> 16) | (v << sh));
+                    pend[2 * l + u] = ld_u64_gpu(box2 + pwd[2 * l + u]);       // unconditional: nothing waits on it
+                }
             }
         };
         if (total > 1) locate(1);
@@ -685,15 +709,15 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 const unsigned long long *box = my_box + (size_t)((g + 1) % CV_D) * CV_MBW;
                 const unsigned tag = (unsigned)(g + 1);
 #pragma unroll
-                for (int u = 0; u < 2; ++u)
+                for (int u = 0; u < 4; ++u)
                     if (pok[u]) {
                         unsigned long long w = pend[u];
                         if ((unsigned)(w >> 32) != tag) w = poll_tag(box + pwd[u], tag, p.status);
                         sm.xs[pxi[u]] = __uint_as_float((unsigned)w);
                     }
-                if (pn > 2) {                                        // rare: several lines arrive
+                if (pn > 4) {                                        // rare: more than two lines arrive
                     const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
-                    for (int k0 = 2; k0 < pn; k0 += 4) {
+                    for (int k0 = 4; k0 < pn; k0 += 4) {
                         unsigned long long w[4];
                         int xi[4], wd[4];
                         bool ok[4];
