@@ -298,6 +298,8 @@ struct LaneCache {
     int lq, lg;                   // rr0 * qp + colofs,  rr0 * Wq + colofs
 };
 
+__device__ void help_handoff(Smem &sm, const CParams &p, int g, unsigned help, int warp, int lane);
+
 // A run of steps [g, g_end) that share the window edge S, for one compute warp.
 template <int S, int KR, int WQ>
 __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache &lc, int &g, int g_end, float c,
@@ -336,6 +338,10 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
                                    sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
                                    c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, CV_NCW * 32, warp, lane);
         }
+        {
+            const unsigned help = (unsigned)sm.desc[g % CV_DR].f >> 16;
+            if (help) help_handoff(sm, p, g, help << 16, warp, lane);
+        }
         if (warp == 0 && lane == 0) CV_STAMP(1);
         CV_STEP_BARRIER();
         if (warp == 0 && lane == 0) CV_STAMP(0);
@@ -356,6 +362,10 @@ __device__ __forceinline__ void run_steps_big(Smem &sm, const CParams &p, int s,
             project_generic<G>(sm, sm.geo[v0.x & 15], s, 1, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
                                sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
                                c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, 0, warp, lane);
+        {
+            const unsigned help = (unsigned)sm.desc[g % CV_DR].f >> 16;
+            if (help) help_handoff(sm, p, g, help << 16, warp, lane);
+        }
         CV_STEP_BARRIER();
     }
 }
@@ -396,7 +406,18 @@ __device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first
         d.qbase = (unsigned)((g % CV_NST) * (CV_PW * CV_PW) + (ex.w0 - ex.e0)) | (g < p.F ? 0x80000000u : 0u);
         const unsigned long long goff = frame_off_q + (unsigned long long)f * plane + (unsigned)(ey.w0 * p.Wq + ex.w0);
         d.goff_lo = (unsigned)goff; d.goff_hi = (unsigned)(goff >> 32);
-        d.f = f; d.run_left = min(fam.run_left, total - g);
+        // bit 16: the departures of step g-1 have more than two lines, bit 17: so have the arrivals of step g+1:
+        // then the compute warps share those lines during step g (changes of window edge move boundaries far)
+        unsigned help = 0;
+        if (g > 0) {
+            const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
+            if (py.R > py.L && px.R > px.L && (px.D - px.L) + (px.R > px.D ? py.D - py.L : 0) > 2) help |= 1u << 16;
+        }
+        if (g + 1 < total) {
+            const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
+            if (ny.R > ny.L && nx.R > nx.L && (nx.R - nx.A) + (nx.A > nx.L ? ny.R - ny.A : 0) > 2) help |= 1u << 17;
+        }
+        d.f = (int)((unsigned)f | help); d.run_left = min(fam.run_left, total - g);
         d.tma_col = ex.e0;
         d.tma_row = (f * p.B_total + frame) * p.H + ey.w0;
         d.tma_k = (g >= p.F && n_items > 0) ? (ey.e1 + 7) >> 3 : 0;          // the first sweep reads no q (q = 0)
@@ -475,6 +496,72 @@ __device__ __forceinline__ int arrival_chunks(const AxisEntry &Y, const AxisEntr
     return 2 * ((X.R - X.A) + (X.A > X.L ? Y.R - Y.A : 0));
 }
 
+// Changes of window edge move the boundaries by up to CV_SD pixels: many lines change owner in one step.  The
+// sender / receiver warps handle the first two lines of every step; the compute warps share the others
+// (line 2 + warp, + CV_NCW, ...) during the step in which they are due.
+__device__ __noinline__ void help_handoff(Smem &sm, const CParams &p, int g, unsigned help, int warp, int lane)
+{
+    const int cta = blockIdx.x;
+    const int bl = cta / (p.NR * p.NC);
+    const int t2 = cta - bl * p.NR * p.NC;
+    const int ci = t2 / p.NC, cj = t2 - ci * p.NC;
+    if (help & (1u << 16)) {                                         // departures of step g-1, tagged g
+        const int cjl = (cj + p.NC - 1) % p.NC, ciu = (ci + p.NR - 1) % p.NR;
+        unsigned long long *const box_l = p.mbox + (size_t)((bl * p.NR + ci) * p.NC + cjl) * CV_D * CV_MBW;
+        unsigned long long *const box_u = p.mbox + (size_t)((bl * p.NR + ciu) * p.NC + cj) * CV_D * CV_MBW;
+        unsigned long long *const box_ul = p.mbox + (size_t)((bl * p.NR + ciu) * p.NC + cjl) * CV_D * CV_MBW;
+        const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
+        const int slot = (g % CV_D) * CV_MBW;
+        const unsigned long long tag = (unsigned long long)(unsigned)g << 32;
+        const int ncl = px.D - px.L, nlines = ncl + (px.R > px.D ? py.D - py.L : 0);
+        for (int line = 2 + warp; line < nlines; line += CV_NCW) {
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int pos = (u << 5) + lane;
+                int r, c, word;
+                bool ok;
+                unsigned long long *box;
+                if (line < ncl) {
+                    c = px.L + line; r = py.L + pos;
+                    ok = r < py.R;
+                    word = mbox_col_word(r, c);
+                    box = (r < py.D) ? box_ul : box_l;
+                } else {
+                    r = py.L + (line - ncl); c = px.D + pos;
+                    ok = c < px.R;
+                    word = mbox_row_word(r, c);
+                    box = box_u;
+                }
+                if (ok) st_u64_gpu(box + slot + word, tag | __float_as_uint(sm.xs[tidx(r, c)]));
+            }
+        }
+    }
+    if (help & (1u << 17)) {                                         // arrivals of step g+1
+        const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
+        const unsigned long long *box = p.mbox + ((size_t)cta * CV_D + (size_t)((g + 1) % CV_D)) * CV_MBW;
+        const unsigned tag = (unsigned)(g + 1);
+        const int nchunks = arrival_chunks(ny, nx);
+        for (int k0 = 4 + 2 * warp; k0 < nchunks; k0 += 2 * CV_NCW) {
+            unsigned long long w[2];
+            int xi[2], wd[2];
+            bool ok[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                int r, c;
+                ok[u] = arrival_chunk(ny, nx, k0 + u, lane, r, c, wd[u]);
+                xi[u] = tidx(r, c);
+                w[u] = ok[u] ? ld_u64_gpu(box + wd[u]) : 0ull;
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+                if (ok[u]) {
+                    if ((unsigned)(w[u] >> 32) != tag) w[u] = poll_tag(box + wd[u], tag, p.status);
+                    sm.xs[xi[u]] = __uint_as_float((unsigned)w[u]);
+                }
+        }
+    }
+}
+
 template <int WQ>
 __global__ void __launch_bounds__(CV_NT, 1)
 conveyor_kernel(const __grid_constant__ CParams p)
@@ -523,7 +610,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
         lc.geom = -1; lc.nwin = 0; lc.rr0 = lc.colofs = lc.lq = lc.lg = 0;
         int g = 0;
         while (g < total) {
-            const int f = sm.desc[g % CV_DR].f;
+            const int f = sm.desc[g % CV_DR].f & 0xffff;
             const int g_end = g + sm.desc[g % CV_DR].run_left;
             const CFamily fam = sm.fams[f];
             switch (fam.side) {
@@ -594,13 +681,13 @@ conveyor_kernel(const __grid_constant__ CParams p)
         for (int g = 0; g < total; ++g) {
             if (g > 0) {
                 if ((g & 3) == 1 && lane >= 1 && lane <= 3) {
-                    // Ring slots g .. g+3 must have been read by the receiver: its counter must have reached
-                    // g + 3 - CV_D.  The counter is re-read only when the ring is half used, and the value is
+                    // Ring slots g .. g+4 (through the next check, so that helpers may send right away) must have
+                    // been read by the receiver: its counter must have reached g + 4 - CV_D.  The counter is re-read only when the ring is half used, and the value is
                     // picked up 4 steps later: the load never sits on this warp's critical path.
                     if (prog_iter >= 0) { prog_seen = max(prog_seen, prog_pend); prog_iter = -1; }
-                    if ((int)prog_seen + CV_D < g + 3) {
-                        prog_seen = poll_prog(my_nbr_prog, (unsigned)(g + 3 - CV_D), p.status);
-                    } else if ((int)prog_seen + CV_D / 2 < g + 3) {
+                    if ((int)prog_seen + CV_D < g + 4) {
+                        prog_seen = poll_prog(my_nbr_prog, (unsigned)(g + 4 - CV_D), p.status);
+                    } else if ((int)prog_seen + CV_D / 2 < g + 4) {
                         prog_pend = ld_u32_gpu(my_nbr_prog);
                         prog_iter = g;
                     }
@@ -641,37 +728,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
                         }
                     }
                 }
-                if (nchunks > 4) {                                   // rare: more than two lines depart
-                    const AxisEntry py = sm.tab[(g - 1) % CV_TR][0], px = sm.tab[(g - 1) % CV_TR][1];
-                    const int ncl = px.D - px.L;
-                    for (int k0 = 4; k0 < nchunks; k0 += 2) {
-                        unsigned long long *dst[2];
-                        float val[2];
-                        bool ok[2];
-#pragma unroll
-                        for (int u = 0; u < 2; ++u) {
-                            const int line = (k0 >> 1), pos = (u << 5) + lane;
-                            int r, c, word;
-                            unsigned long long *box;
-                            if (line < ncl) {
-                                c = px.L + line; r = py.L + pos;
-                                ok[u] = r < py.R;
-                                word = mbox_col_word(r, c);
-                                box = (r < py.D) ? box_ul : box_l;
-                            } else {
-                                r = py.L + (line - ncl); c = px.D + pos;
-                                ok[u] = c < px.R;
-                                word = mbox_row_word(r, c);
-                                box = box_u;
-                            }
-                            dst[u] = box + slot + word;
-                            val[u] = ok[u] ? sm.xs[tidx(r, c)] : 0.0f;
-                        }
-#pragma unroll
-                        for (int u = 0; u < 2; ++u)
-                            if (ok[u]) st_u64_gpu(dst[u], tag | __float_as_uint(val[u]));
-                    }
-                }
+                // (lines beyond the second are sent by the compute warps: help_handoff)
             }
             if (lane == 0) CV_STAMP(4);
             CV_STEP_BARRIER();
@@ -715,27 +772,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
                         if ((unsigned)(w >> 32) != tag) w = poll_tag(box + pwd[u], tag, p.status);
                         sm.xs[pxi[u]] = __uint_as_float((unsigned)w);
                     }
-                if (pn > 4) {                                        // rare: more than two lines arrive
-                    const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
-                    for (int k0 = 4; k0 < pn; k0 += 4) {
-                        unsigned long long w[4];
-                        int xi[4], wd[4];
-                        bool ok[4];
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            int r, c;
-                            ok[u] = (k0 + u < pn) && arrival_chunk(ny, nx, k0 + u, lane, r, c, wd[u]);
-                            xi[u] = tidx(r, c);
-                            w[u] = ok[u] ? ld_u64_gpu(box + wd[u]) : 0ull;
-                        }
-#pragma unroll
-                        for (int u = 0; u < 4; ++u)
-                            if (ok[u]) {
-                                if ((unsigned)(w[u] >> 32) != tag) w[u] = poll_tag(box + wd[u], tag, p.status);
-                                sm.xs[xi[u]] = __uint_as_float((unsigned)w[u]);
-                            }
-                    }
-                }
+                // (lines beyond the second are received by the compute warps: help_handoff)
                 __syncwarp();
                 if (lane == 0) CV_STAMP(2);
                 if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // step g+1 has been read
