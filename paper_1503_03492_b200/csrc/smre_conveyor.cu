@@ -172,7 +172,7 @@ struct Smem {
     float qs[CV_NST * CV_PW * CV_PW];        // q stages, filled by TMA: [(row - first window row) * qp + (column - c0)], c0 = first window column rounded down to 4
     AxisEntry tab[CV_TR][2];                 // [step % CV_TR][0 = y, 1 = x]
     StepDesc desc[CV_DR];                    // [step % CV_DR]
-    GeomDesc geo[16];                        // [geom & 15]
+    GeomDesc geo[CV_DR];                     // [geom % CV_DR]: at most CV_AHEAD + CV_BATCH ids are planned ahead
     unsigned long long qbar[CV_NST];         // mbarriers: the TMA box of a stage has landed
     CFamily fams[CV_MAX_F];
     int abort;                               // set by the receiver warp when the failure flag is up
@@ -313,7 +313,7 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
         const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g % CV_DR].geom);
         if (warp == 0 && lane == 0) CV_STAMP(6);
         if ((int)v0.x != lc.geom) {                            // rare: the tile's window counts changed
-            const GeomDesc ge = sm.geo[v0.x & 15];
+            const GeomDesc ge = sm.geo[v0.x % CV_DR];
             const int n_items = (int)v0.y;
             lc.geom = (int)v0.x;
             const int item = warp * 32 + lane;
@@ -334,7 +334,7 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
             float *qg = p.q + (((unsigned long long)v1.y << 32) | v1.x) + lc.lg;
             project_item<S, KR, G, WQ>(sm.xs, qs0, qg, tidx(r0, cc), lc.nwin, c, sqrt_c, p.Wq, p.qp, (v0.w >> 31) != 0);
             if ((int)v0.y > CV_NCW * 32)
-                project_generic<G>(sm, sm.geo[v0.x & 15], S, KR, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
+                project_generic<G>(sm, sm.geo[v0.x % CV_DR], S, KR, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
                                    sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
                                    c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, CV_NCW * 32, warp, lane);
         }
@@ -359,7 +359,7 @@ __device__ __forceinline__ void run_steps_big(Smem &sm, const CParams &p, int s,
         const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g % CV_DR].geom);
         const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g % CV_DR].goff_lo);
         if ((int)v0.y > 0)
-            project_generic<G>(sm, sm.geo[v0.x & 15], s, 1, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
+            project_generic<G>(sm, sm.geo[v0.x % CV_DR], s, 1, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
                                sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
                                c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, 0, warp, lane);
         {
@@ -397,7 +397,7 @@ __device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first
     const int my_geom = geom + __popc(chg & (0xffffffffu >> (31 - lane)));
     if (changed) {
         GeomDesc ge; ge.nwx = ex.nw; ge.nwy = ey.nw; ge.n_items = n_items; ge.pad = 0;
-        sm.geo[my_geom & 15] = ge;
+        sm.geo[my_geom % CV_DR] = ge;
     }
     if (on) {
         StepDesc d;

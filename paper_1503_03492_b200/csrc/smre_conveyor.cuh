@@ -36,7 +36,7 @@ struct AxisEntry {
 
 // Vertically stacked windows handled by one lane of the conveyor kernel, per window edge (the kernel's
 // template instantiations and the planner's e0 must agree on this).
-__host__ __device__ constexpr int cv_kr(int side) { return side == 1 ? 8 : side == 2 ? 4 : side == 3 ? 3 : side <= 5 ? 2 : 1; }
+__host__ __device__ constexpr int cv_kr(int side) { return side == 1 ? 5 : side == 2 ? 3 : side <= 5 ? 2 : 1; }
 static_assert(sizeof(AxisEntry) == 16, "AxisEntry must be 16 bytes");
 
 // Tile-boundary trajectories of one axis for `total` steps.
