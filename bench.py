@@ -228,9 +228,24 @@ def run_gpu(args, w, rank, world):
                     "algorithmic_bytes_per_step": nums["bytes_per_step"],
                     "note": "achieved = dense-model bytes of one whole step (all launches of the step) / "
                             "CUDA-event time of the step; see DESIGN.md sec. 7"}
+        if w.variant == "standard" and launch[0] == smre.SMRE_SCHED_PERSISTENT and w.name.startswith("C1") \
+                and w.n_sweeps == 200:
+            # dram__bytes_read.sum + dram__bytes_write.sum of this launch from the committed ncu --set full
+            # capture (profiles/r01_ncu_full_conveyor_c1_metrics.txt): 39.487 GB + 41.020 GB
+            roofline["traffic"] = 80.507e9
+            roofline["traffic_source"] = "profiles/r01_ncu_full_conveyor_c1_metrics.txt"
         if w.variant != "standard":
-            roofline["note"] = ("ICD is bound by fp32 issue, not HBM (DESIGN.md sec. 7); the HBM fraction is "
-                                "reported so that nobody reads it as a bandwidth result")
+            # ICD keeps q in registers: it is bound by fp32 issue, not by HBM.  Model: 5 fp32
+            # lane-instructions (add, fma, mul, sub, select) per pixel per level pass per inner cycle.
+            _, _, sm_max = measured_peaks()
+            lane_instr = 5.0 * w.n_sweeps * nums["families"] * w.batch * w.H * w.W
+            peak_alu = 148 * 128 * sm_max * 1e6
+            roofline = {"bound": "alu", "achieved": lane_instr / per_launch_s / 1e12, "peak": peak_alu / 1e12,
+                        "unit": "T lane-instr/s", "frac": lane_instr / per_launch_s / peak_alu, "traffic": None,
+                        "kernel": kernel, "hbm_frac": achieved / peak,
+                        "note": "fp32 issue model: 5 lane-instructions per pixel per level pass per cycle; peak = "
+                                "148 SMs x 128 lanes x sm_max_mhz; hbm_frac is reported so that nobody reads ICD "
+                                "as a bandwidth result"}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             sample_sweeps = max(1, min(w.n_sweeps, args.ref_sweeps))
@@ -244,7 +259,7 @@ def run_gpu(args, w, rank, world):
             "config": {"workload": w.name, "note": w.note, "variant": w.variant, "n_sweeps": w.n_sweeps,
                        "H": w.H, "W": w.W, "batch": w.batch, "families": nums["families"],
                        "windows_per_sweep": nums["windows_per_sweep"],
-                       "schedule": {1: "graph", 2: "conveyor"}.get(launch[0], str(launch[0])),
+                       "schedule": ("icd_shifts" if w.variant != "standard" else {1: "graph", 2: "conveyor"}.get(launch[0], str(launch[0]))),
                        "tiles": [launch[2], launch[3]],
                        "l2": "q planes (>L2) re-zeroed every step" if flush is None else "256 MiB flush between steps",
                        "parallelism": "replicas only" if world > 1 else "1 GPU"},
