@@ -23,7 +23,11 @@ __device__ __forceinline__ float ball_scale(float n2, float c, float sqrt_c) {
     (void)sqrt_c;
     return (n2 > c) ? __fsqrt_rn(__fdiv_rn(c, n2)) : 1.0f;
 #else
-    return (n2 > c) ? sqrt_c * rsqrtf(n2) : 1.0f;
+    // rsqrt.approx.ftz: the bare MUFU.RSQ.  rsqrtf() wraps it in a denormal rescue that can never trigger
+    // here (the branch is only taken for n2 > c > 0, far from the denormal range) but sits on the chain.
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(n2));
+    return (n2 > c) ? sqrt_c * r : 1.0f;
 #endif
 }
 

@@ -186,6 +186,12 @@ struct Smem {
         if ((g & 7) == 7 && *(volatile int *)&sm.abort) return;                   \
     } while (0)
 
+#if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 2
+#define CV_CLK(k) do { if (clk) clk[k] = clock64(); } while (0)
+#else
+#define CV_CLK(k) ((void)0)
+#endif
+
 #ifdef SMRE_CV_TRACE_BUILD
 #define CV_STAMP(slot)                                                            \
     do {                                                                          \
@@ -204,7 +210,8 @@ struct Smem {
 // xor-shuffle tree over the G lanes of the window.
 template <int S, int KR, int G, int WQ>
 __device__ __forceinline__ void project_item(float *xs, const float *qs0, float *__restrict__ qg, int xi0,
-                                             int nwin, float c, float sqrt_c, int Wq_rt, int qp_rt, bool first_sweep)
+                                             int nwin, float c, float sqrt_c, int Wq_rt, int qp_rt, bool first_sweep,
+                                             long long *clk = nullptr)
 {
     constexpr int R = S * KR;
     const int Wq = WQ ? WQ : Wq_rt;
@@ -224,13 +231,16 @@ __device__ __forceinline__ void project_item(float *xs, const float *qs0, float 
             part[k] = fmaf(v[rr], v[rr], part[k]);
         }
     }
+    if (part[0] >= 0.0f) CV_CLK(3);
 #pragma unroll
     for (int m = G / 2; m > 0; m >>= 1)
 #pragma unroll
         for (int k = 0; k < KR; ++k) part[k] += __shfl_xor_sync(0xffffffffu, part[k], m);
+    if (part[0] >= 0.0f) CV_CLK(4);
 #pragma unroll
     for (int k = 0; k < KR; ++k) {
         const float alpha = ball_scale(part[k], c, sqrt_c);
+        if (alpha >= 0.0f) CV_CLK(5);
 #pragma unroll
         for (int r = 0; r < S; ++r) {
             const int rr = k * S + r;
@@ -310,7 +320,17 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
     const int Wq = WQ ? WQ : p.Wq;
     const int qp = WQ ? CV_PW : p.qp;
     for (; g < g_end; ++g) {
+#if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 2
+        long long clkbuf[8];
+        long long *clk = (warp == 0 && lane == 0 && p.trace) ? clkbuf : nullptr;
+        if (clk) for (int i = 0; i < 8; ++i) clk[i] = 0;
+        CV_CLK(0);
+#else
+        long long *clk = nullptr;
+#endif
         const uint4 v0 = *reinterpret_cast<const uint4 *>(&sm.desc[g % CV_DR].geom);
+        const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g % CV_DR].goff_lo);
+        if ((int)v0.y >= 0) CV_CLK(1);
         if (warp == 0 && lane == 0) CV_STAMP(6);
         if ((int)v0.x != lc.geom) {                            // rare: the tile's window counts changed
             const GeomDesc ge = sm.geo[v0.x % CV_DR];
@@ -328,23 +348,29 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
             lc.lg = lc.rr0 * Wq + lc.colofs;
         }
         if (lc.busy) {
-            const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g % CV_DR].goff_lo);
             const int r0 = (int)(v0.z & 0xffffu) + lc.rr0, cc = (int)(v0.z >> 16) + lc.colofs;
-            const float *qs0 = sm.qs + (v0.w & 0x7fffffffu) + lc.lq;
+            const float *qs0 = sm.qs + (v0.w & 0x1fffffffu) + lc.lq;
             float *qg = p.q + (((unsigned long long)v1.y << 32) | v1.x) + lc.lg;
-            project_item<S, KR, G, WQ>(sm.xs, qs0, qg, tidx(r0, cc), lc.nwin, c, sqrt_c, p.Wq, p.qp, (v0.w >> 31) != 0);
+            if (r0 + cc >= 0) CV_CLK(2);
+            project_item<S, KR, G, WQ>(sm.xs, qs0, qg, tidx(r0, cc), lc.nwin, c, sqrt_c, p.Wq, p.qp, (v0.w >> 31) != 0, clk);
+            CV_CLK(6);
             if ((int)v0.y > CV_NCW * 32)
                 project_generic<G>(sm, sm.geo[v0.x % CV_DR], S, KR, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
-                                   sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
+                                   sm.qs + (v0.w & 0x1fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
                                    c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, CV_NCW * 32, warp, lane);
         }
-        {
-            const unsigned help = (unsigned)sm.desc[g % CV_DR].f >> 16;
-            if (help) help_handoff(sm, p, g, help << 16, warp, lane);
-        }
+        if (v0.w & 0x60000000u) help_handoff(sm, p, g, (v0.w >> 13) & 0x30000u, warp, lane);
         if (warp == 0 && lane == 0) CV_STAMP(1);
+        CV_CLK(7);
         CV_STEP_BARRIER();
         if (warp == 0 && lane == 0) CV_STAMP(0);
+#if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 2
+        if (clk) {
+            const long long t_end = clock64();
+            for (int i = 1; i < 8; ++i) p.trace[((size_t)cta * total + g) * 8 + i] = (unsigned long long)(clk[i] - clk[0]);
+            p.trace[((size_t)cta * total + g) * 8] = (unsigned long long)(t_end - clk[0]);
+        }
+#endif
     }
 }
 
@@ -360,12 +386,9 @@ __device__ __forceinline__ void run_steps_big(Smem &sm, const CParams &p, int s,
         const uint2 v1 = *reinterpret_cast<const uint2 *>(&sm.desc[g % CV_DR].goff_lo);
         if ((int)v0.y > 0)
             project_generic<G>(sm, sm.geo[v0.x % CV_DR], s, 1, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
-                               sm.qs + (v0.w & 0x7fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
+                               sm.qs + (v0.w & 0x1fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
                                c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, 0, warp, lane);
-        {
-            const unsigned help = (unsigned)sm.desc[g % CV_DR].f >> 16;
-            if (help) help_handoff(sm, p, g, help << 16, warp, lane);
-        }
+        if (v0.w & 0x60000000u) help_handoff(sm, p, g, (v0.w >> 13) & 0x30000u, warp, lane);
         CV_STEP_BARRIER();
     }
 }
@@ -403,7 +426,7 @@ __device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first
         StepDesc d;
         d.geom = my_geom; d.n_items = n_items;
         d.w0yx = ey.w0 | (ex.w0 << 16);
-        d.qbase = (unsigned)((g % CV_NST) * (CV_PW * CV_PW) + (ex.w0 - ex.e0)) | (g < p.F ? 0x80000000u : 0u);
+        d.qbase = (unsigned)((g % CV_NST) * (CV_PW * CV_PW) + (ex.w0 - ex.e0)) | (g < p.F ? 0x80000000u : 0u);   // bits 29, 30: help flags, below
         const unsigned long long goff = frame_off_q + (unsigned long long)f * plane + (unsigned)(ey.w0 * p.Wq + ex.w0);
         d.goff_lo = (unsigned)goff; d.goff_hi = (unsigned)(goff >> 32);
         // bit 16: the departures of step g-1 have more than two lines, bit 17: so have the arrivals of step g+1:
@@ -417,7 +440,8 @@ __device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first
             const AxisEntry ny = sm.tab[(g + 1) % CV_TR][0], nx = sm.tab[(g + 1) % CV_TR][1];
             if (ny.R > ny.L && nx.R > nx.L && (nx.R - nx.A) + (nx.A > nx.L ? ny.R - ny.A : 0) > 2) help |= 1u << 17;
         }
-        d.f = (int)((unsigned)f | help); d.run_left = min(fam.run_left, total - g);
+        d.f = f; d.run_left = min(fam.run_left, total - g);
+        d.qbase |= help << 13;                                        // bits 29 (send), 30 (receive)
         d.tma_col = ex.e0;
         d.tma_row = (f * p.B_total + frame) * p.H + ey.w0;
         d.tma_k = (g >= p.F && n_items > 0) ? (ey.e1 + 7) >> 3 : 0;          // the first sweep reads no q (q = 0)
@@ -610,7 +634,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
         lc.geom = -1; lc.nwin = 0; lc.rr0 = lc.colofs = lc.lq = lc.lg = 0;
         int g = 0;
         while (g < total) {
-            const int f = sm.desc[g % CV_DR].f & 0xffff;
+            const int f = sm.desc[g % CV_DR].f;
             const int g_end = g + sm.desc[g % CV_DR].run_left;
             const CFamily fam = sm.fams[f];
             switch (fam.side) {
@@ -992,6 +1016,7 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
     p.NR = pl->NR; p.NC = pl->NC; p.qp = pl->qp;
     memcpy(p.qmap, pl->qmap, sizeof p.qmap);
     const int tiles = pl->NR * pl->NC;
+    if ((e = cudaMemsetAsync(pl->d_status, 0, sizeof(int), st)) != cudaSuccess) return e;   // health flag of THIS run
     const char *trace_path = getenv("SMRE_CV_TRACE");        // debug only: synchronises and writes a file
     if (trace_path && cudaMalloc(&p.trace, (size_t)tiles * p.total * 64) != cudaSuccess) p.trace = nullptr;
     for (int f0 = 0; f0 < pl->B; f0 += pl->frames_per_launch) {
