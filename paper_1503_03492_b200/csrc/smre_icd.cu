@@ -20,16 +20,20 @@ __device__ __forceinline__ int morton_even_bits(int t) {   // bits 0,2,4 of t ->
     return (t & 1) | ((t >> 1) & 2) | ((t >> 2) & 4);
 }
 
-template <int K>
+// Pixel block per lane (LP = log2 of its edge): 4x4 is the throughput choice (fewest shuffles per pixel);
+// 2x2 gives four times the lanes and a shorter dependent chain per level pass, which wins when the whole
+// problem is too small to fill the machine (C2: 512^2, K = 3).  Tiles of 16x16 and 32x32 need 4x4 (a tile
+// must fit in two warps).
+template <int K, int LP>
 __global__ void __launch_bounds__(128)
 icd_shift_kernel(const float *src, float *dst, int H, int W, int org,
                  int nty, int ntx, long long n_tiles, int smin, IcdLevels lv, int n_cycles)
 {
     constexpr int L = 1 << K;
-    constexpr int P = L < 4 ? L : 4;              // pixel block edge per lane
+    constexpr int P = 1 << LP;                    // pixel block edge per lane: 1, 2, 2, 2, 4, 4
     constexpr int NB = L / P;                     // blocks per tile edge
-    constexpr int LPT = NB * NB;                  // lanes per tile: 1, 1, 1, 4, 16, 64
-    constexpr int KIN = K < 2 ? K : 2;            // highest level reduced inside a lane
+    constexpr int LPT = NB * NB;                  // lanes per tile: 1, 1, 4, 16, 16, 64
+    constexpr int KIN = K < LP ? K : LP;          // highest level reduced inside a lane
     constexpr int NP = P * P;
 
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -109,7 +113,7 @@ icd_shift_kernel(const float *src, float *dst, int H, int W, int org,
                     v[p] = x[p] + q[k][p];
                     part = fmaf(v[p], v[p], part);
                 }
-                const int lanes = 1 << (2 * (k - 2));             // 4, 16, 64
+                const int lanes = 1 << (2 * (k - LP));            // 4, 16, 64
 #pragma unroll
                 for (int m = 1; m < 32; m <<= 1)
                     if (m < lanes) part += __shfl_xor_sync(0xffffffffu, part, m);
@@ -169,12 +173,12 @@ icd_shift_kernel(const float *src, float *dst, int H, int W, int org,
                 dst[frame + (size_t)(gy0 + r) * W + (gx0 + c)] = x[r * P + c];
 }
 
-template <int K>
-static cudaError_t launch_k(const float *src, float *dst, int B, int H, int W, int shift_i,
-                            const IcdLevels &lv, int n_cycles, cudaStream_t st)
+template <int K, int LP>
+static cudaError_t launch_kp(const float *src, float *dst, int B, int H, int W, int shift_i,
+                             const IcdLevels &lv, int n_cycles, cudaStream_t st)
 {
     constexpr int L = 1 << K;
-    constexpr int P = L < 4 ? L : 4;
+    constexpr int P = 1 << LP;
     constexpr int LPT = (L / P) * (L / P);
     const int o = (1 << shift_i) % L;
     const int org = o ? o - L : 0;
@@ -183,9 +187,22 @@ static cudaError_t launch_k(const float *src, float *dst, int B, int H, int W, i
     const long long lanes = n_tiles * LPT;
     const int threads = 128;
     const long long blocks = (lanes + threads - 1) / threads;
-    icd_shift_kernel<K><<<(unsigned)blocks, threads, 0, st>>>(src, dst, H, W, org, nty, ntx, n_tiles,
+    icd_shift_kernel<K, LP><<<(unsigned)blocks, threads, 0, st>>>(src, dst, H, W, org, nty, ntx, n_tiles,
                                                              shift_i, lv, n_cycles);
     return cudaGetLastError();
+}
+
+template <int K>
+static cudaError_t launch_k(const float *src, float *dst, int B, int H, int W, int shift_i,
+                            const IcdLevels &lv, int n_cycles, cudaStream_t st)
+{
+    constexpr int LPmax = K < 2 ? K : 2;                   // 4x4 blocks where the tile allows it
+    if constexpr (K == 2 || K == 3) {
+        // lanes the 4x4 layout would give; below about half a machine of resident threads use 2x2 blocks
+        const long long lanes4 = (long long)B * ((H + (1 << K) - 1) >> K) * ((W + (1 << K) - 1) >> K) * (1 << (2 * (K - 2)));
+        if (lanes4 < 148ll * 1024) return launch_kp<K, 1>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
+    }
+    return launch_kp<K, LPmax>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
 }
 
 cudaError_t launch_icd_shift(const float *src, float *dst, int B, int H, int W, int K, int shift_i,
