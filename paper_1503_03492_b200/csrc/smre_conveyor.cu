@@ -319,6 +319,9 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
     constexpr int LG = S <= 1 ? 0 : S <= 2 ? 1 : S <= 4 ? 2 : 3;
     const int Wq = WQ ? WQ : p.Wq;
     const int qp = WQ ? CV_PW : p.qp;
+    // Items go to compute warps 15, 0, 1, 2, ...: with four schedulers (warp % 4) the usual 9-13 busy warps
+    // then spread 3-3-3-x over them together with the control, sender and receiver warps (16, 17, 18).
+    const int cwi = (warp + 1) % CV_NCW;
     for (; g < g_end; ++g) {
 #if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 2
         long long clkbuf[8];
@@ -336,12 +339,12 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
             const GeomDesc ge = sm.geo[v0.x % CV_DR];
             const int n_items = (int)v0.y;
             lc.geom = (int)v0.x;
-            const int item = warp * 32 + lane;
+            const int item = cwi * 32 + lane;
             const int grp = item >> LG, j = item & (G - 1);
             const int by = ge.nwx > 0 ? grp / ge.nwx : 0, wix = grp - by * ge.nwx;
             const bool on = item < n_items && j < S;
             lc.nwin = on ? min(KR, ge.nwy - by * KR) : 0;
-            lc.busy = warp * 32 < n_items;
+            lc.busy = cwi * 32 < n_items;
             lc.rr0 = by * KR * S;
             lc.colofs = wix * S + j;
             lc.lq = lc.rr0 * qp + lc.colofs;
@@ -357,7 +360,7 @@ __device__ __forceinline__ void run_steps(Smem &sm, const CParams &p, LaneCache 
             if ((int)v0.y > CV_NCW * 32)
                 project_generic<G>(sm, sm.geo[v0.x % CV_DR], S, KR, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
                                    sm.qs + (v0.w & 0x1fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
-                                   c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, CV_NCW * 32, warp, lane);
+                                   c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, CV_NCW * 32, cwi, lane);
         }
         if (v0.w & 0x60000000u) help_handoff(sm, p, g, (v0.w >> 13) & 0x30000u, warp, lane);
         if (warp == 0 && lane == 0) CV_STAMP(1);
@@ -387,7 +390,7 @@ __device__ __forceinline__ void run_steps_big(Smem &sm, const CParams &p, int s,
         if ((int)v0.y > 0)
             project_generic<G>(sm, sm.geo[v0.x % CV_DR], s, 1, (int)(v0.z & 0xffffu), (int)(v0.z >> 16),
                                sm.qs + (v0.w & 0x1fffffffu), p.q + (((unsigned long long)v1.y << 32) | v1.x),
-                               c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, 0, warp, lane);
+                               c, sqrt_c, Wq, qp, (v0.w >> 31) != 0, 0, (warp + 1) % CV_NCW, lane);
         if (v0.w & 0x60000000u) help_handoff(sm, p, g, (v0.w >> 13) & 0x30000u, warp, lane);
         CV_STEP_BARRIER();
     }
