@@ -71,8 +71,9 @@ typedef enum {
  *   c_table  (host, in)   n_sides thresholds c_S > 0, c_table[a] belongs to sides[a].
  *   variant               SMRE_INCOMPLETE needs every 2^k, k <= floor(log2(max side)), in sides[];
  *                         other sides are ignored by it.
- * Allocates (device): SMRE_STANDARD  sum(side^2)*batch*H*W*4 bytes of increment planes plus a
- * batch*H*W*4 work image and a small mailbox workspace; SMRE_INCOMPLETE nothing of image size.
+ * Allocates (device): SMRE_STANDARD  sum(side^2)*batch*H*Wq*4 bytes of increment planes (Wq = W rounded up
+ * to a multiple of 4) plus a batch*H*W*4 work image and, if the conveyor can tile the problem, its mailboxes
+ * (256 KiB per tile) and boundary tables; SMRE_INCOMPLETE nothing of image size.
  * The arrays sides / c_table are copied; the caller may free them on return.
  */
 smre_status smre_create(smre_handle *out, int H, int W, int batch,
@@ -83,7 +84,9 @@ smre_status smre_create(smre_handle *out, int H, int W, int batch,
  * Project.  y_dev, x_out_dev: DEVICE pointers to batch*H*W contiguous fp32.  y_dev is only read;
  * x_out_dev == y_dev (in place) is allowed (the paper's kernels work in place on e,
  * PAPER.md:516).  n_sweeps >= 1: sweeps (standard) / inner cycles per shift (incomplete).
- * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous.
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous, with one exception: the first
+ * call of a handle with a given n_sweeps under the conveyor schedule plans the tile boundaries on the host
+ * and uploads the tables (a few ms, cached per n_sweeps), which synchronises with the stream once.
  */
 smre_status smre_project(smre_handle h, const float *y_dev, float *x_out_dev,
                          int n_sweeps, void *cuda_stream);

@@ -12,8 +12,14 @@
 //     neighbour: dependencies point ONE way, the left / upper tiles simply run a few steps behind
 //     the right / lower ones, and the hand-off latency is off the critical path;
 //   * x lives in shared memory (torus-addressed 64 x 64 tile per CTA) from the first to the last
-//     step; q streams HBM -> shared memory (16-byte cp.async.cg, CV_PF steps ahead; its addresses
+//     step; q streams HBM -> shared memory (one TMA box per step, CV_PF steps ahead: its addresses
 //     do not depend on x) -> registers -> HBM (streaming stores).  That is the only HBM traffic.
+// Warp roles per CTA: CV_NCW compute warps (one lane = one column of cv_kr(side) stacked windows; one
+// template instantiation per window edge, entered once per run of equal edges), a control warp (plans
+// CV_BATCH steps at a time, one per lane, into a descriptor ring; per step it orders the TMA box of step
+// g + CV_PF and waits for the box of step g + 1), a sender warp and a receiver warp (first two lines of
+// every hand-off, located by the planner; the compute warps share the rest at changes of window edge).
+// One bar.sync per step.
 // Hand-off: the previous owner writes each departing pixel as ONE 8-byte word {step tag, value} into
 // the new owner's mailbox (global memory, L2 resident, ring of CV_D steps); the new owner loads the
 // words one step before it needs them and deposits them into its tile.  No fences, no flags: the tag
@@ -53,6 +59,7 @@ struct CParams {
     int F, total;
     int H, W, Wq, B_total, frame0;   // Wq: row pitch of the q planes (W rounded up to 4)
     int NR, NC;
+    int pace;                     // steps an empty slot may run ahead of the slot that will feed it
     int qp;                       // row pitch (floats) of a q stage in shared memory = columns of a TMA box
     CUtensorMap qmap[8];          // q as a 2-D tensor [F*B*H rows][Wq]; box = qp columns x 8*(k+1) rows
 };
@@ -472,6 +479,8 @@ __device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first
                 }
                 a = wbase | (xbase << 16);
                 b = var0 | (len << 8) | (sh << 16) | (k == 0 ? (unsigned)chunks << 24 : 0u);
+                if (arr && k == 1 && ex.R <= ex.L) b |= 0x80000000u;                // no tile column in this slot now
+                if (arr && k == 1 && ey.R <= ey.L) b |= 0x40000000u;                // no tile row in this slot now
             };
             unsigned x0, x1;
             line(true, 0, d.recv_a[0], d.recv_b[0], x0);
@@ -765,6 +774,12 @@ conveyor_kernel(const __grid_constant__ CParams p)
         // The first line (two chunks) of every step -- all there is in the usual step -- is located and
         // requested one step ahead; its geometry is kept in registers for the deposit a step later.
         unsigned long long *const my_box = p.mbox + (size_t)cta * CV_D * CV_MBW;
+        // A slot without a tile has no hand-off to wait for and would race ahead of the pipeline; its q boxes
+        // (ordered CV_PF steps ahead) would then be read before the previous sweep has written them.  Such a
+        // slot therefore keeps the pace of the neighbour slot its next tile will be fed from.
+        const unsigned *const pace_r = p.prog + (size_t)((bl * p.NR + ci) * p.NC + (cj + 1) % p.NC) * CV_PROG_STRIDE;
+        const unsigned *const pace_d = p.prog + (size_t)((bl * p.NR + (ci + 1) % p.NR) * p.NC + cj) * CV_PROG_STRIDE;
+        unsigned pace_seen = 0;                      // lane 0 / lane 1: last value seen of pace_r / pace_d
         unsigned long long pend[4] = {0, 0, 0, 0};
         int pxi[4] = {0, 0, 0, 0}, pwd[4] = {0, 0, 0, 0}, pn = 0;
         bool pok[4] = {false, false, false, false};
@@ -802,6 +817,16 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 // (lines beyond the second are received by the compute warps: help_handoff)
                 __syncwarp();
                 if (lane == 0) CV_STAMP(2);
+                const unsigned dead = sm.desc[(g + 1) % CV_DR].recv_b[1] >> 30;
+                if (dead) {
+                    // No tile at step g+1.  An unborn column will be fed from the right, an unborn row from below:
+                    // keep that neighbour's pace, at most CParams::pace steps ahead of it (a tight leash costs a
+                    // counter round trip every few steps and, through flow control, slows the live tiles next to it).  Pacing with the OTHER neighbour too would tie the whole row / column of empty
+                    // slots, and through flow control every live tile next to it, to the slowest tile of the grid.
+                    if (lane == 0 && (dead & 2) && p.NC > 1 && (int)pace_seen + p.pace < g) pace_seen = poll_prog(pace_r, (unsigned)(g - p.pace), p.status);
+                    if (lane == 1 && (dead & 1) && p.NR > 1 && (int)pace_seen + p.pace < g) pace_seen = poll_prog(pace_d, (unsigned)(g - p.pace), p.status);
+                    __syncwarp();
+                }
                 if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // step g+1 has been read
                 if (g + 2 < total) locate(g + 2);
             }
@@ -847,6 +872,7 @@ struct ConveyorPlan {
     int H, W, Wq, B, F;
     int T_y, T_x, NR, NC;
     int frames_per_launch;
+    int pace = CV_PACE_MAX;
     ConveyorKernel kernel;
     int qp = 0;                         // columns of a TMA box = row pitch of a q stage
     CUtensorMap qmap[8];
@@ -898,6 +924,8 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
     if (fams.empty() || (int)fams.size() > CV_MAX_F || H > 32000 || W > 32000) return nullptr;
     // q of a step is fetched CV_PF steps ahead of its use and was written one sweep (F steps) earlier
     if ((int)fams.size() < CV_PF + 3) return nullptr;
+    int smax_f = 1;
+    for (const Family &f : fams) smax_f = std::max(smax_f, f.side);
     if ((long long)fams.size() * B * H >= (1ll << 31)) return nullptr;          // tensor rows are 32-bit coordinates
     int dev = 0, n_sm = 0, smem_optin = 0, coop = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
@@ -920,11 +948,21 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
     char why[160];
     // the tiling is chosen on a short run; tables_for() re-plans (and re-verifies) each real length
     if (!conveyor_summary(H, W, fams, 3, capacity, &cs, why, sizeof why)) return nullptr;
+    // With several tiles the q of a pixel is written by one CTA and read, one sweep (F steps) later, by a CTA
+    // up / left of it, CV_PF steps ahead of its use.  Along y a consumer may run up to `side` steps ahead of
+    // its producer between two row hand-offs, ownership moves by at most two tiles per sweep, and an empty slot
+    // may run `pace` steps ahead of the slot that feeds it: the write is certainly visible if a sweep is longer
+    // than all of this together.  (One tile: no such constraint.)
+    int pace = CV_PACE_MAX;
+    if (cs.tiles_y * cs.tiles_x > 1) {
+        pace = std::min(CV_PACE_MAX, (int)fams.size() - (CV_PF + 4 * smax_f + 16));
+        if (pace < 8) return nullptr;
+    }
 
     ConveyorPlan *pl = new ConveyorPlan;
     pl->H = H; pl->W = W; pl->Wq = (W + 3) & ~3; pl->B = B; pl->F = (int)fams.size();
     pl->T_y = cs.T_y; pl->T_x = cs.T_x; pl->NR = cs.tiles_y; pl->NC = cs.tiles_x;
-    pl->fams = fams; pl->q = q; pl->xwork = xwork; pl->kernel = kernel;
+    pl->fams = fams; pl->q = q; pl->xwork = xwork; pl->kernel = kernel; pl->pace = pace;
     {   // q as a 2-D fp32 tensor [F*B*H][Wq]; one map per box height 8, 16, .., 64 (plain layout, zero fill)
         typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -1016,7 +1054,7 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
     p.y = y; p.x_out = x_out; p.q = pl->q; p.fams = pl->d_fams; p.taby = tabs->d_y; p.tabx = tabs->d_x;
     p.mbox = pl->d_mbox; p.prog = pl->d_prog; p.status = pl->d_status;
     p.F = pl->F; p.total = pl->F * n_sweeps; p.H = pl->H; p.W = pl->W; p.Wq = pl->Wq; p.B_total = pl->B;
-    p.NR = pl->NR; p.NC = pl->NC; p.qp = pl->qp;
+    p.NR = pl->NR; p.NC = pl->NC; p.qp = pl->qp; p.pace = pl->pace;
     memcpy(p.qmap, pl->qmap, sizeof p.qmap);
     const int tiles = pl->NR * pl->NC;
     if ((e = cudaMemsetAsync(pl->d_status, 0, sizeof(int), st)) != cudaSuccess) return e;   // health flag of THIS run

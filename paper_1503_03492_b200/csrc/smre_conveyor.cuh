@@ -1,5 +1,5 @@
-// Interface of the conveyor sweep scheduler (smre_conveyor_plan.cpp-style host planner in
-// smre_conveyor_plan.cu, kernel in smre_conveyor.cu).  See DESIGN.md sec. 5 for the idea:
+// Interface of the conveyor sweep scheduler (host planner in smre_conveyor_plan.cu, kernel and launch in
+// smre_conveyor.cu).  See DESIGN.md sec. 6.2 for the idea:
 // tile boundaries MOVE so that at every family step they lie on that family's window grid; no
 // window ever straddles a tile boundary, pixels change owner in one direction only (to the left /
 // upper neighbour), and the neighbour latency is off the critical path.
@@ -22,6 +22,7 @@ constexpr int CV_BATCH = 16;            // the control warp plans this many step
 constexpr int CV_AHEAD = 8;             // ... starting this many steps ahead of the step it runs in
 constexpr int CV_MBW = 2 * CV_SD * CV_PW;   // 8-byte words per mailbox slot
 constexpr int CV_PROG_STRIDE = 64;       // progress counters 256 bytes apart: no line is shared by two CTAs
+constexpr int CV_PACE_MAX = 64;          // an empty slot may run at most this many steps ahead of the slot that feeds it
 constexpr int CV_MAX_F = 1024;          // families kept in shared memory
 
 // One axis of one tile slot at one step (16 bytes).  All positions are clipped to [0, N].

@@ -70,6 +70,26 @@ def test_conveyor_repeatable():
         sol.close()
 
 
+# ---- several tiles, short sweeps: q written by one CTA is read a sweep later by another one ------------------
+@pytest.mark.parametrize("H,W,B,sides,n", [(160, 176, 2, [1, 2, 3, 4], 4), (128, 128, 1, [1, 2, 3, 4], 5),
+                                           (200, 200, 1, [1, 2, 3, 4, 5, 6], 3), (256, 256, 2, list(range(1, 9)), 2),
+                                           (96, 300, 1, [2, 3, 5], 4)])
+def test_conveyor_tiles_match_graph_bitwise(H, W, B, sides, n):
+    rng = np.random.default_rng(H + W)
+    y = (1.6 * rng.standard_normal((B, H, W))).astype(np.float32)
+    y[:, : H // 2, : W // 2] += 1.5
+    c = si.thresholds(sides)
+    ref, _ = gpu_project(y, sides, c, "standard", n, smre.SMRE_SCHED_GRAPH)
+    for _ in range(3):
+        try:
+            x, launch = gpu_project(y, sides, c, "standard", n, smre.SMRE_SCHED_PERSISTENT)
+        except smre.SmreError as e:
+            assert e.status == smre.smre.SMRE_EUNSUPPORTED
+            pytest.skip("conveyor does not take this problem")
+        assert launch[2] * launch[3] > 1
+        assert np.array_equal(x, ref)
+
+
 # ---- small, ragged, degenerate --------------------------------------------------------------------
 CASES = [
     # H, W, batch, sides, variant, sweeps
@@ -78,6 +98,7 @@ CASES = [
     (33, 35, 1, [7, 8], "standard", 9),
     (40, 72, 2, [16, 5], "standard", 4),
     (70, 66, 1, [32, 17, 2], "standard", 3),              # largest compiled side
+    (160, 176, 2, [1, 2, 3, 4], "standard", 4),           # conveyor: 11 x 12 tiles, two frames (one launch each)
     (8, 8, 1, [8], "standard", 3),                        # one window = the image
     (5, 7, 1, [1], "standard", 2),                        # clip only
     (50, 61, 1, [1, 2, 4, 8], "incomplete", 11),          # ragged ICD, K = 3
