@@ -261,7 +261,8 @@ def run_gpu(args, w, rank, world):
                        "windows_per_sweep": nums["windows_per_sweep"],
                        "schedule": ("icd_shifts" if w.variant != "standard" else {1: "graph", 2: "conveyor"}.get(launch[0], str(launch[0]))),
                        "tiles": [launch[2], launch[3]],
-                       "l2": "q planes (>L2) re-zeroed every step" if flush is None else "256 MiB flush between steps",
+                       "l2": ("q planes (204 MiB for C1, > 126 MB L2) are rewritten by every step: nothing of a step survives "
+                              "in L2 for the next one") if flush is None else "256 MiB flush between steps",
                        "parallelism": "replicas only" if world > 1 else "1 GPU"},
             "window_projections_per_s": value * nums["windows_per_sweep"],
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(y_pin.numel() * 4),
@@ -286,7 +287,7 @@ def main():
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1)")
     ap.add_argument("--n-sweeps", type=int, default=None, help="override the config's sweep count (debug)")
     ap.add_argument("--schedule", default="auto", choices=["auto", "graph", "persistent", "conveyor"])
-    ap.add_argument("--ref-sweeps", type=int, default=50, help="oracle sample size in sweeps (~15 s on C1)")
+    ap.add_argument("--ref-sweeps", type=int, default=200, help="oracle sample size in sweeps (~12 s on C1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
