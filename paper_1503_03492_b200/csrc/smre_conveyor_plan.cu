@@ -106,11 +106,17 @@ bool plan_axis(int N, const std::vector<Family> &fams, bool y_axis, int n_sweeps
             live += clipN(ceil_grid(a + (k + 1) * T, o, s), N) > clipN(ceil_grid(a + k * T, o, s), N);
         max_live = std::max(max_live, live);
     }
-    out.slots = max_live;
     out.drift = anchor[total - 1];
 
     // ---- pass 2: the table ----------------------------------------------------------------------
-    const int S = out.slots;
+    // A slot must stay EMPTY for at least one step between the death of its tile at the far edge and the
+    // birth of its next tile at the near edge.  A CTA walks through the steps in order; if it were the last
+    // tile of the chain at step g and the first one at step g+1, the hand-off of step g would close a cycle
+    // (every tile finishes step g only after it has received what its neighbour produced in step g).
+    // One spare slot breaks the cycle.
+    for (int S = max_live; S <= max_live + 1; ++S) {
+    out.slots = S;
+    out.max_extent = 0; out.max_move = 0;
     out.tab.assign((size_t)total * S, AxisEntry{});
     for (int g = 0; g < total; ++g) {
         const int s = side(g), o = off(g), ag = anchor[g];
@@ -140,6 +146,14 @@ bool plan_axis(int N, const std::vector<Family> &fams, bool y_axis, int n_sweeps
             dst = e;
             out.max_extent = std::max(out.max_extent, R - L);
         }
+    }
+    bool switched = false;                                 // a slot alive in two consecutive steps with different tiles
+    for (int g = 0; g + 1 < total && !switched; ++g)
+        for (int c = 0; c < S; ++c) {
+            const AxisEntry &e = out.tab[(size_t)g * S + c], &n = out.tab[(size_t)(g + 1) * S + c];
+            if (e.R > e.L && n.R > n.L && n.A == n.L) { switched = true; break; }
+        }
+    if (!switched) break;
     }
     return verify_axis(out, why, why_len);
 }
@@ -182,6 +196,7 @@ bool verify_axis(const AxisPlan &ap, char *why, size_t why_len)
         for (int c = 0; c < S; ++c) {
             const AxisEntry &e = E(g, c), &n = E(g + 1, c);
             const bool live = e.R > e.L, nlive = n.R > n.L;
+            if (live && nlive && n.A == n.L && S > 1) { set_why(why, why_len, "step %d slot %d: a new tile right after the old one (no empty step)", g, c); return false; }
             // (2) what the tile keeps is exactly what it holds, un-arrived, at the next step
             if (live && e.D < e.R) {
                 if (!nlive || n.L != e.D || n.A != e.R) { set_why(why, why_len, "step %d slot %d: kept part does not continue", g, c); return false; }

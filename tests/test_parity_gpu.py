@@ -73,7 +73,11 @@ def test_conveyor_repeatable():
 # ---- several tiles, short sweeps: q written by one CTA is read a sweep later by another one ------------------
 @pytest.mark.parametrize("H,W,B,sides,n", [(160, 176, 2, [1, 2, 3, 4], 4), (128, 128, 1, [1, 2, 3, 4], 5),
                                            (200, 200, 1, [1, 2, 3, 4, 5, 6], 3), (256, 256, 2, list(range(1, 9)), 2),
-                                           (96, 300, 1, [2, 3, 5], 4)])
+                                           (96, 300, 1, [2, 3, 5], 4),
+                                           # a tile row / column that dies at the far edge one step before the same CTA
+                                           # slot would host the newborn one at the near edge (needs the spare slot)
+                                           (113, 88, 1, [8, 7, 6, 5, 4, 3, 2, 1], 3), (160, 175, 1, [6, 8, 3], 3),
+                                           (407, 71, 2, [1, 2, 3, 4, 5, 6, 7], 3), (384, 97, 1, [4, 5, 6, 7, 8], 3)])
 def test_conveyor_tiles_match_graph_bitwise(H, W, B, sides, n):
     rng = np.random.default_rng(H + W)
     y = (1.6 * rng.standard_normal((B, H, W))).astype(np.float32)
@@ -88,6 +92,30 @@ def test_conveyor_tiles_match_graph_bitwise(H, W, B, sides, n):
             pytest.skip("conveyor does not take this problem")
         assert launch[2] * launch[3] > 1
         assert np.array_equal(x, ref)
+
+
+def test_conveyor_random_shapes_match_graph_bitwise():
+    rng = np.random.default_rng(2024)
+    pools = [list(range(1, 9)), list(range(1, 7)), [2, 3, 5, 7], [1, 3, 5, 6, 8], [4, 5, 6, 7, 8], [8, 7, 6, 5, 4, 3, 2, 1]]
+    ran = 0
+    for _ in range(40):
+        H, W = int(rng.integers(65, 420)), int(rng.integers(65, 420))
+        B, n = int(rng.integers(1, 3)), int(rng.integers(2, 4))
+        sides = pools[int(rng.integers(len(pools)))]
+        y = (1.6 * rng.standard_normal((B, H, W))).astype(np.float32)
+        y[:, : H // 2, : W // 2] += 1.5
+        c = si.thresholds(sides)
+        try:
+            x, launch = gpu_project(y, sides, c, "standard", n, smre.SMRE_SCHED_PERSISTENT)
+        except smre.SmreError as e:
+            assert e.status == smre.smre.SMRE_EUNSUPPORTED, (H, W, B, sides, n, str(e))
+            continue
+        ref, _ = gpu_project(y, sides, c, "standard", n, smre.SMRE_SCHED_GRAPH)
+        assert np.array_equal(x, ref), (H, W, B, sides, n, launch)
+        ran += 1
+        if ran >= 12:
+            break
+    assert ran >= 6
 
 
 # ---- small, ragged, degenerate --------------------------------------------------------------------

@@ -39,3 +39,9 @@ def test_bad_arguments():
         with pytest.raises(smre.SmreError) as e:
             smre.smre_plan_check(*args)
         assert e.value.status == smre.smre.SMRE_EINVAL
+
+
+def test_spare_slot_when_death_and_birth_touch():
+    # 113 = 7 * 16 + 1: the one-row tile at the bottom dies in the step before the same slot would be born at the top
+    ty, tx, *_ = smre.smre_plan_check(113, 88, [8, 7, 6, 5, 4, 3, 2, 1], 3)
+    assert (ty, tx) == (9, 7)
