@@ -59,7 +59,9 @@ struct CParams {
     int F, total;
     int H, W, Wq, B_total, frame0;   // Wq: row pitch of the q planes (W rounded up to 4)
     int NR, NC;
-    int pace;                     // steps an empty slot may run ahead of the slot that will feed it
+    unsigned *gmin;               // per frame of the launch: a lower bound of all its progress counters (see `lead`)
+    int lead;                     // no slot runs more than this many steps ahead of gmin: F - CV_PF - 3
+    int gmin_mask;                // gmin is refreshed every gmin_mask + 1 steps (4 .. 16, about lead / 4)
     int qp;                       // row pitch (floats) of a q stage in shared memory = columns of a TMA box
     CUtensorMap qmap[8];          // q as a 2-D tensor [F*B*H rows][Wq]; box = qp columns x 8*(k+1) rows
 };
@@ -122,6 +124,24 @@ __device__ __noinline__ unsigned long long poll_tag(const unsigned long long *p,
         }
     }
     return v;
+}
+// A slot held back by gmin: the published value is refreshed only every few steps of the slot that keeps it, and
+// that slot may be waiting (through hand-offs) for this one.  So the lane recomputes the minimum itself, and
+// publishes it, until it suffices: a slot is held back only while it really is `lead` steps ahead of some slot.
+__device__ __noinline__ unsigned poll_gmin(const unsigned *counters, int n, unsigned *gmin, unsigned need, int *status) {
+    const long long t0 = clock64();
+    for (unsigned spins = 1;; ++spins) {
+        unsigned m = 0xffffffffu;
+#pragma unroll 8
+        for (int i = 0; i < n; ++i) m = min(m, ld_u32_gpu(counters + (size_t)i * CV_PROG_STRIDE));
+        atomicMax(gmin, m);                                // never lower a published bound (see publish_min)
+        if (m >= need) return m;
+        __nanosleep(400);
+        if ((spins & 63u) == 0) {
+            if (*(volatile int *)status != 0) return need;
+            if (clock64() - t0 > 2000000000LL) { atomicExch(status, 1); return need; }
+        }
+    }
 }
 __device__ __noinline__ unsigned poll_prog(const unsigned *p, unsigned need, int *status) {
     const long long t0 = clock64();
@@ -479,8 +499,6 @@ __device__ __forceinline__ void plan_steps(Smem &sm, const CParams &p, int first
                 }
                 a = wbase | (xbase << 16);
                 b = var0 | (len << 8) | (sh << 16) | (k == 0 ? (unsigned)chunks << 24 : 0u);
-                if (arr && k == 1 && ex.R <= ex.L) b |= 0x80000000u;                // no tile column in this slot now
-                if (arr && k == 1 && ey.R <= ey.L) b |= 0x40000000u;                // no tile row in this slot now
             };
             unsigned x0, x1;
             line(true, 0, d.recv_a[0], d.recv_b[0], x0);
@@ -714,7 +732,34 @@ conveyor_kernel(const __grid_constant__ CParams p)
         const unsigned *my_nbr_prog = p.prog + (size_t)nbr_cta(lane >= 1 && lane <= 3 ? lane : 1) * CV_PROG_STRIDE;
         unsigned prog_pend = 0, prog_seen = 0;  // lanes 1..3: progress of the receiving CTAs
         int prog_iter = -1;                     // step at which prog_pend was requested (-1: none in flight)
+        // The sender warp of the first slot of a frame also keeps that frame's gmin: every few steps it reads all
+        // progress counters of the frame (requested two steps before they are used) and publishes their minimum.
+        const int tiles = p.NR * p.NC;
+        const bool keeper = tiles > 1 && ci == 0 && cj == 0;
+        const unsigned *const frame_prog = p.prog + (size_t)bl * tiles * CV_PROG_STRIDE;
+        unsigned *const gmin_out = p.gmin + (size_t)bl * CV_PROG_STRIDE;
+        unsigned cnt[5] = {0, 0, 0, 0, 0};
+        auto read_counters = [&]() {
+#pragma unroll
+            for (int k = 0; k < 5; ++k) {
+                const int i = lane + 32 * k;
+                cnt[k] = i < tiles ? ld_u32_gpu(frame_prog + (size_t)i * CV_PROG_STRIDE) : 0xffffffffu;
+            }
+        };
+        auto publish_min = [&]() {
+            unsigned m = min(min(min(cnt[0], cnt[1]), min(cnt[2], cnt[3])), cnt[4]);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
+            // atomicMax: this minimum may be older than one the receiver lane of this CTA has published while it
+            // was held back; a bound that drops could hold back the very slot this one is waiting for
+            if (lane == 0) atomicMax(gmin_out, m);
+            return m;
+        };
         for (int g = 0; g < total; ++g) {
+            if (keeper) {
+                if ((g & p.gmin_mask) == 0) read_counters();
+                else if ((g & p.gmin_mask) == 2) publish_min();
+            }
             if (g > 0) {
                 if ((g & 3) == 1 && lane >= 1 && lane <= 3) {
                     // Ring slots g .. g+4 (through the next check, so that helpers may send right away) must have
@@ -769,17 +814,34 @@ conveyor_kernel(const __grid_constant__ CParams p)
             if (lane == 0) CV_STAMP(4);
             CV_STEP_BARRIER();
         }
+        if (keeper) {
+            // slower slots still need gmin: keep it until every counter has its final value (total - 1)
+            const long long t0 = clock64();
+            for (;;) {
+                read_counters();
+                if (publish_min() + 1 >= (unsigned)total || *(volatile int *)p.status != 0) break;
+                if (clock64() - t0 > 4000000000LL) { atomicExch(p.status, 1); break; }
+                __nanosleep(500);
+            }
+        }
     } else {
         // =============== receiver warp: arrivals of step g+1 into the tile ================================
         // The first line (two chunks) of every step -- all there is in the usual step -- is located and
         // requested one step ahead; its geometry is kept in registers for the deposit a step later.
         unsigned long long *const my_box = p.mbox + (size_t)cta * CV_D * CV_MBW;
-        // A slot without a tile has no hand-off to wait for and would race ahead of the pipeline; its q boxes
-        // (ordered CV_PF steps ahead) would then be read before the previous sweep has written them.  Such a
-        // slot therefore keeps the pace of the neighbour slot its next tile will be fed from.
-        const unsigned *const pace_r = p.prog + (size_t)((bl * p.NR + ci) * p.NC + (cj + 1) % p.NC) * CV_PROG_STRIDE;
-        const unsigned *const pace_d = p.prog + (size_t)((bl * p.NR + (ci + 1) % p.NR) * p.NC + cj) * CV_PROG_STRIDE;
-        unsigned pace_seen = 0;                      // lane 0 / lane 1: last value seen of pace_r / pace_d
+        // The q of a pixel is written by one slot and read, a sweep (F steps) later, by a slot up / left of it,
+        // which orders the box CV_PF steps ahead of its use.  Hand-offs alone do not order the two: a boundary that
+        // does not move for some steps carries no message, and a slot without a tile waits for nothing.  So no
+        // slot runs more than `lead` = F - CV_PF - 3 steps ahead of gmin, a lower bound of every counter of
+        // the frame: the box of step g is ordered in iteration g - CV_PF, after the check of iteration
+        // g - CV_PF - 1, when every counter was >= g - CV_PF - 1 - lead = g - F + 2, i.e. every slot had issued the
+        // q writes of step g - F (a counter value v is stored after the barrier of step v - 2).  The natural lag
+        // of the pipeline is far smaller than a sweep of the usual configurations, so the check is almost free:
+        // gmin is re-read (a step before the value is needed) only when the last value seen gets old.
+        const unsigned *const gmin_ptr = p.gmin + (size_t)bl * CV_PROG_STRIDE;
+        unsigned gm_seen = 0, gm_pend = 0;           // lane 2
+        bool gm_inflight = false;
+        const bool paced = p.NR * p.NC > 1;
         unsigned long long pend[4] = {0, 0, 0, 0};
         int pxi[4] = {0, 0, 0, 0}, pwd[4] = {0, 0, 0, 0}, pn = 0;
         bool pok[4] = {false, false, false, false};
@@ -817,14 +879,14 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 // (lines beyond the second are received by the compute warps: help_handoff)
                 __syncwarp();
                 if (lane == 0) CV_STAMP(2);
-                const unsigned dead = sm.desc[(g + 1) % CV_DR].recv_b[1] >> 30;
-                if (dead) {
-                    // No tile at step g+1.  An unborn column will be fed from the right, an unborn row from below:
-                    // keep that neighbour's pace, at most CParams::pace steps ahead of it (a tight leash costs a
-                    // counter round trip every few steps and, through flow control, slows the live tiles next to it).  Pacing with the OTHER neighbour too would tie the whole row / column of empty
-                    // slots, and through flow control every live tile next to it, to the slowest tile of the grid.
-                    if (lane == 0 && (dead & 2) && p.NC > 1 && (int)pace_seen + p.pace < g) pace_seen = poll_prog(pace_r, (unsigned)(g - p.pace), p.status);
-                    if (lane == 1 && (dead & 1) && p.NR > 1 && (int)pace_seen + p.pace < g) pace_seen = poll_prog(pace_d, (unsigned)(g - p.pace), p.status);
+                if (paced) {                                   // q ordering: at most `lead` steps ahead of gmin
+                    if (lane == 2) {
+                        if (gm_inflight) { gm_seen = max(gm_seen, gm_pend); gm_inflight = false; }
+                        else if ((int)gm_seen + p.lead < g + 8) { gm_pend = ld_u32_gpu(gmin_ptr); gm_inflight = true; }
+                        if ((int)gm_seen + p.lead < g)        // held back: work out the minimum itself, it may be stale
+                            gm_seen = poll_gmin(p.prog + (size_t)bl * p.NR * p.NC * CV_PROG_STRIDE, p.NR * p.NC,
+                                                p.gmin + (size_t)bl * CV_PROG_STRIDE, (unsigned)(g - p.lead), p.status);
+                    }
                     __syncwarp();
                 }
                 if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // step g+1 has been read
@@ -872,7 +934,6 @@ struct ConveyorPlan {
     int H, W, Wq, B, F;
     int T_y, T_x, NR, NC;
     int frames_per_launch;
-    int pace = CV_PACE_MAX;
     ConveyorKernel kernel;
     int qp = 0;                         // columns of a TMA box = row pitch of a q stage
     CUtensorMap qmap[8];
@@ -948,21 +1009,16 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
     char why[160];
     // the tiling is chosen on a short run; tables_for() re-plans (and re-verifies) each real length
     if (!conveyor_summary(H, W, fams, 3, capacity, &cs, why, sizeof why)) return nullptr;
-    // With several tiles the q of a pixel is written by one CTA and read, one sweep (F steps) later, by a CTA
-    // up / left of it, CV_PF steps ahead of its use.  Along y a consumer may run up to `side` steps ahead of
-    // its producer between two row hand-offs, ownership moves by at most two tiles per sweep, and an empty slot
-    // may run `pace` steps ahead of the slot that feeds it: the write is certainly visible if a sweep is longer
-    // than all of this together.  (One tile: no such constraint.)
-    int pace = CV_PACE_MAX;
-    if (cs.tiles_y * cs.tiles_x > 1) {
-        pace = std::min(CV_PACE_MAX, (int)fams.size() - (CV_PF + 4 * smax_f + 16));
-        if (pace < 8) return nullptr;
-    }
+    // With several tiles a slot may lead the slowest slot by F - CV_PF - 3 steps (q ordering, see the receiver
+    // warp); the pipeline wants some slack per tile to hide the latency of a hand-off.
+    // The tile that feeds another is at least one step ahead of it, so the last tile leads the first by the
+    // length of the chain between them; a lead with no slack beyond that would run, but in lock step.
+    if (cs.tiles_y * cs.tiles_x > 1 && (int)fams.size() - CV_PF - 3 < cs.tiles_y + cs.tiles_x + 4) return nullptr;
 
     ConveyorPlan *pl = new ConveyorPlan;
     pl->H = H; pl->W = W; pl->Wq = (W + 3) & ~3; pl->B = B; pl->F = (int)fams.size();
     pl->T_y = cs.T_y; pl->T_x = cs.T_x; pl->NR = cs.tiles_y; pl->NC = cs.tiles_x;
-    pl->fams = fams; pl->q = q; pl->xwork = xwork; pl->kernel = kernel; pl->pace = pace;
+    pl->fams = fams; pl->q = q; pl->xwork = xwork; pl->kernel = kernel;
     {   // q as a 2-D fp32 tensor [F*B*H][Wq]; one map per box height 8, 16, .., 64 (plain layout, zero fill)
         typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -1003,7 +1059,7 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
     const bool good =
         cudaMalloc(&pl->d_fams, cf.size() * sizeof(CFamily)) == cudaSuccess &&
         cudaMalloc(&pl->d_mbox, pl->mbox_bytes) == cudaSuccess &&
-        cudaMalloc(&pl->d_prog, n_cta * CV_PROG_STRIDE * sizeof(unsigned)) == cudaSuccess &&
+        cudaMalloc(&pl->d_prog, (n_cta + pl->frames_per_launch) * CV_PROG_STRIDE * sizeof(unsigned)) == cudaSuccess &&
         cudaMalloc(&pl->d_status, sizeof(int)) == cudaSuccess &&
         cudaMemcpy(pl->d_fams, cf.data(), cf.size() * sizeof(CFamily), cudaMemcpyHostToDevice) == cudaSuccess &&
         cudaMemset(pl->d_status, 0, sizeof(int)) == cudaSuccess;
@@ -1054,7 +1110,9 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
     p.y = y; p.x_out = x_out; p.q = pl->q; p.fams = pl->d_fams; p.taby = tabs->d_y; p.tabx = tabs->d_x;
     p.mbox = pl->d_mbox; p.prog = pl->d_prog; p.status = pl->d_status;
     p.F = pl->F; p.total = pl->F * n_sweeps; p.H = pl->H; p.W = pl->W; p.Wq = pl->Wq; p.B_total = pl->B;
-    p.NR = pl->NR; p.NC = pl->NC; p.qp = pl->qp; p.pace = pl->pace;
+    p.NR = pl->NR; p.NC = pl->NC; p.qp = pl->qp; p.lead = pl->F - CV_PF - 3;
+    p.gmin_mask = p.lead >= 64 ? 15 : p.lead >= 32 ? 7 : 3;
+    p.gmin = pl->d_prog + (size_t)pl->frames_per_launch * pl->NR * pl->NC * CV_PROG_STRIDE;
     memcpy(p.qmap, pl->qmap, sizeof p.qmap);
     const int tiles = pl->NR * pl->NC;
     if ((e = cudaMemsetAsync(pl->d_status, 0, sizeof(int), st)) != cudaSuccess) return e;   // health flag of THIS run
@@ -1065,7 +1123,7 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
         const int nb = std::min(pl->frames_per_launch, pl->B - f0);
         // tags and progress counters restart in every launch
         if ((e = cudaMemsetAsync(pl->d_mbox, 0, (size_t)nb * tiles * CV_D * CV_MBW * 8, st)) != cudaSuccess) return e;
-        if ((e = cudaMemsetAsync(pl->d_prog, 0, (size_t)nb * tiles * CV_PROG_STRIDE * sizeof(unsigned), st)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(pl->d_prog, 0, (size_t)pl->frames_per_launch * (tiles + 1) * CV_PROG_STRIDE * sizeof(unsigned), st)) != cudaSuccess) return e;
         void *args[] = {&p};
         e = cudaLaunchCooperativeKernel((const void *)pl->kernel, dim3((unsigned)(nb * tiles)),
                                         dim3(CV_NT), args, sizeof(Smem), st);

@@ -22,7 +22,6 @@ constexpr int CV_BATCH = 16;            // the control warp plans this many step
 constexpr int CV_AHEAD = 8;             // ... starting this many steps ahead of the step it runs in
 constexpr int CV_MBW = 2 * CV_SD * CV_PW;   // 8-byte words per mailbox slot
 constexpr int CV_PROG_STRIDE = 64;       // progress counters 256 bytes apart: no line is shared by two CTAs
-constexpr int CV_PACE_MAX = 64;          // an empty slot may run at most this many steps ahead of the slot that feeds it
 constexpr int CV_MAX_F = 1024;          // families kept in shared memory
 
 // One axis of one tile slot at one step (16 bytes).  All positions are clipped to [0, N].
@@ -48,6 +47,7 @@ struct AxisPlan {
     int max_extent = 0;                // largest R - L
     int max_move = 0;                  // largest boundary movement in one step (inside the image)
     long long drift = 0;               // total anchor movement
+    int reach = 0;                     // largest slot distance from the reader of a q value to its writer one sweep earlier
     std::vector<AxisEntry> tab;        // [total][slots]
 };
 
@@ -73,7 +73,7 @@ cudaError_t conveyor_run(ConveyorPlan *p, const float *y, float *x_out, int n_sw
 
 // Host-only planning summary for tests / diagnostics (no device needed).
 struct ConveyorSummary {
-    int tiles_y, tiles_x, T_y, T_x, max_h, max_w, max_move_y, max_move_x;
+    int tiles_y, tiles_x, T_y, T_x, max_h, max_w, max_move_y, max_move_x, reach_y, reach_x;
     long long drift_y, drift_x, table_bytes;
 };
 bool conveyor_summary(int H, int W, const std::vector<Family> &fams, int n_sweeps, int max_ctas,

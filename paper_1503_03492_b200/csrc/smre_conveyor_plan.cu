@@ -155,6 +155,22 @@ bool plan_axis(int N, const std::vector<Family> &fams, bool y_axis, int n_sweeps
         }
     if (!switched) break;
     }
+    // How far (in slots, cyclically to the right / down) the slot that wrote the increment of a pixel in one
+    // sweep is from the slot that reads it in the next: the owner of a pixel moves to lower tile numbers only,
+    // and the owner number is monotone in the pixel, so the last pixel of a tile has the farthest writer.
+    out.reach = 0;
+    {
+        const int S = out.slots, F = (int)fams.size();
+        for (int g = F; g < total; ++g)
+            for (int c = 0; c < S; ++c) {
+                const AxisEntry &e = out.tab[(size_t)g * S + c];
+                if (e.R <= e.L) continue;
+                for (int d = out.reach + 1; d < S; ++d) {
+                    const AxisEntry &w = out.tab[(size_t)(g - F) * S + (c + d) % S];
+                    if (w.R > w.L && w.L < e.R && w.R > e.L) out.reach = d;
+                }
+            }
+    }
     return verify_axis(out, why, why_len);
 }
 
@@ -245,7 +261,7 @@ bool conveyor_summary(int H, int W, const std::vector<Family> &fams, int n_sweep
     int smax = 1;
     for (const Family &f : fams) smax = std::max(smax, f.side);
     if ((int)fams.size() > CV_MAX_F) { set_why(why, why_len, "more than %d families", CV_MAX_F); return false; }
-    struct Cand { int T, slots, ext, move; long long drift; };
+    struct Cand { int T, slots, ext, move, reach; long long drift; };
     std::vector<Cand> cy, cx;
     char w2[160];
     for (int axis = 0; axis < 2; ++axis) {
@@ -253,7 +269,7 @@ bool conveyor_summary(int H, int W, const std::vector<Family> &fams, int n_sweep
         for (int T : candidates(N, smax)) {
             AxisPlan ap;
             if (!plan_axis(N, fams, axis == 0, n_sweeps, T, ap, w2, sizeof w2)) continue;
-            (axis == 0 ? cy : cx).push_back(Cand{T, ap.slots, ap.max_extent, ap.max_move, ap.drift});
+            (axis == 0 ? cy : cx).push_back(Cand{T, ap.slots, ap.max_extent, ap.max_move, ap.reach, ap.drift});
         }
     }
     if (cy.empty() || cx.empty()) { set_why(why, why_len, "no admissible tiling of an axis (last reason: %d)", 0); if (why && why_len) snprintf(why, why_len, "no admissible tiling: %s", w2); return false; }
@@ -270,7 +286,7 @@ bool conveyor_summary(int H, int W, const std::vector<Family> &fams, int n_sweep
     if (out) {
         const int F = (int)fams.size();
         *out = ConveyorSummary{cy[by].slots, cx[bx].slots, cy[by].T, cx[bx].T, cy[by].ext, cx[bx].ext,
-                               cy[by].move, cx[bx].move, cy[by].drift, cx[bx].drift,
+                               cy[by].move, cx[bx].move, cy[by].reach, cx[bx].reach, cy[by].drift, cx[bx].drift,
                                (long long)F * n_sweeps * (cy[by].slots + cx[bx].slots) * (long long)sizeof(AxisEntry)};
     }
     return true;

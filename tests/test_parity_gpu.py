@@ -77,7 +77,12 @@ def test_conveyor_repeatable():
                                            # a tile row / column that dies at the far edge one step before the same CTA
                                            # slot would host the newborn one at the near edge (needs the spare slot)
                                            (113, 88, 1, [8, 7, 6, 5, 4, 3, 2, 1], 3), (160, 175, 1, [6, 8, 3], 3),
-                                           (407, 71, 2, [1, 2, 3, 4, 5, 6, 7], 3), (384, 97, 1, [4, 5, 6, 7, 8], 3)])
+                                           (407, 71, 2, [1, 2, 3, 4, 5, 6, 7], 3), (384, 97, 1, [4, 5, 6, 7, 8], 3),
+                                           # q ordering across sweeps: many narrow tiles and a short sweep (a pixel changes
+                                           # owner six times per sweep; window grids that nest, so boundaries often rest and
+                                           # carry no hand-off), chains of empty slots
+                                           (492, 54, 1, [2, 4, 6, 8], 3), (98, 437, 2, [1, 2, 4, 8], 4),
+                                           (142, 553, 2, [1, 2, 4, 8], 2), (187, 447, 3, [1, 2, 4, 8], 3)])
 def test_conveyor_tiles_match_graph_bitwise(H, W, B, sides, n):
     rng = np.random.default_rng(H + W)
     y = (1.6 * rng.standard_normal((B, H, W))).astype(np.float32)
