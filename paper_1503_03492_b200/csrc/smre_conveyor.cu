@@ -59,9 +59,9 @@ struct CParams {
     int F, total;
     int H, W, Wq, B_total, frame0;   // Wq: row pitch of the q planes (W rounded up to 4)
     int NR, NC;
-    unsigned *gmin;               // per frame of the launch: a lower bound of all its progress counters (see `lead`)
-    int lead;                     // no slot runs more than this many steps ahead of gmin: F - CV_PF - 3
-    int gmin_mask;                // gmin is refreshed every gmin_mask + 1 steps (4 .. 16, about lead / 4)
+    unsigned *gmin;               // per frame of the launch: a lower bound of all its progress counters (control warp)
+    int gmin_mask;                // gmin is recomputed every gmin_mask + 1 steps (4 .. 16)
+    int fence_mask;               // the fenced counters it is computed from are refreshed every fence_mask + 1 steps (4 .. 64)
     int qp;                       // row pitch (floats) of a q stage in shared memory = columns of a TMA box
     CUtensorMap qmap[8];          // q as a 2-D tensor [F*B*H rows][Wq]; box = qp columns x 8*(k+1) rows
 };
@@ -73,7 +73,13 @@ __device__ __forceinline__ unsigned long long ld_u64_gpu(const unsigned long lon
     return v;
 }
 __device__ __forceinline__ void st_u64_gpu(unsigned long long *p, unsigned long long v) {
+#if defined(SMRE_CV_EXP) && SMRE_CV_EXP == 7
+    if (v == 0x123456789abcull) asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+#elif defined(SMRE_CV_EXP) && SMRE_CV_EXP == 8
+    asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+#else
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+#endif
 }
 __device__ __forceinline__ unsigned ld_u32_gpu(const unsigned *p) {
     unsigned v;
@@ -127,13 +133,14 @@ __device__ __noinline__ unsigned long long poll_tag(const unsigned long long *p,
 }
 // A slot held back by gmin: the published value is refreshed only every few steps of the slot that keeps it, and
 // that slot may be waiting (through hand-offs) for this one.  So the lane recomputes the minimum itself, and
-// publishes it, until it suffices: a slot is held back only while it really is `lead` steps ahead of some slot.
+// publishes it, until it suffices: a slot is held back only while some slot really is that far behind.
 __device__ __noinline__ unsigned poll_gmin(const unsigned *counters, int n, unsigned *gmin, unsigned need, int *status) {
     const long long t0 = clock64();
     for (unsigned spins = 1;; ++spins) {
         unsigned m = 0xffffffffu;
 #pragma unroll 8
-        for (int i = 0; i < n; ++i) m = min(m, ld_u32_gpu(counters + (size_t)i * CV_PROG_STRIDE));
+        for (int i = 0; i < n; ++i) m = min(m, ld_u32_gpu(counters + (size_t)i * CV_PROG_STRIDE + 1));
+        __threadfence();
         atomicMax(gmin, m);                                // never lower a published bound (see publish_min)
         if (m >= need) return m;
         __nanosleep(400);
@@ -219,7 +226,13 @@ struct Smem {
 #define CV_CLK(k) ((void)0)
 #endif
 
-#ifdef SMRE_CV_TRACE_BUILD
+#if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 4
+#define CV_RCLK(k) do { if (p.trace && lane == 0) rclk[k] = clock64(); } while (0)
+#else
+#define CV_RCLK(k) ((void)0)
+#endif
+
+#if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD != 4
 #define CV_STAMP(slot)                                                            \
     do {                                                                          \
         if (p.trace) {                                                            \
@@ -555,6 +568,9 @@ __device__ __forceinline__ int arrival_chunks(const AxisEntry &Y, const AxisEntr
 // (line 2 + warp, + CV_NCW, ...) during the step in which they are due.
 __device__ __noinline__ void help_handoff(Smem &sm, const CParams &p, int g, unsigned help, int warp, int lane)
 {
+#if defined(SMRE_CV_EXP) && (SMRE_CV_EXP == 3 || SMRE_CV_EXP == 5 || SMRE_CV_EXP == 7 || SMRE_CV_EXP == 9 || SMRE_CV_EXP == 10)
+    return;
+#endif
     const int cta = blockIdx.x;
     const int bl = cta / (p.NR * p.NC);
     const int t2 = cta - bl * p.NR * p.NC;
@@ -687,6 +703,18 @@ conveyor_kernel(const __grid_constant__ CParams p)
         int st1 = 1 % CV_NST;                  // q stage of step g + 1
         int stp = CV_PF % CV_NST;              // q stage of step g + CV_PF
         unsigned phase = 0;                    // bit s: parity the next wait on q stage s has to use
+        // Ordering of q across sweeps.  The q of a pixel is written by one slot and read, a sweep (F steps) later,
+        // by a slot up / left of it, which orders the box CV_PF steps ahead of its use.  Hand-offs alone do not
+        // order the two: a boundary that does not move for some steps carries no message, and a slot without a
+        // tile waits for nothing.  So the box of step s is ordered only when gmin, a lower bound of every progress
+        // (fenced) counter of the frame, has reached s - F + 2: a value v is stored after the barrier of step v - 2
+        // and a fence, so every slot's q writes of step s - F are visible.  The natural lag of the pipeline (tail to
+        // head) is far smaller than a sweep of the usual configurations, and gmin is re-read, a step before the
+        // value is needed, only when the last value seen gets old: the check is almost free.
+        const unsigned *const gmin_ptr = p.gmin + (size_t)bl * CV_PROG_STRIDE;
+        unsigned gm_seen = 0, gm_pend = 0;     // lane 0
+        bool gm_inflight = false;
+        const bool ordered = p.NR * p.NC > 1;
         for (int g = 0; g < total; ++g) {
             if ((g & (CV_BATCH - 1)) == 0) {
                 // table entries of steps [g + 32, g + 48); those fetched 16 steps ago are complete and visible
@@ -700,6 +728,21 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 if (g + CV_PF < total) {                             // order the q box of step g + CV_PF
                     const StepDesc &d = sm.desc[(g + CV_PF) % CV_DR];
                     const int k = d.tma_k;
+                    if (ordered) {
+                        const int need = g + CV_PF - p.F + 2;
+                        bool fresh = false;
+                        if (gm_inflight) { gm_seen = max(gm_seen, gm_pend); gm_inflight = false; fresh = true; }
+                        else if ((int)gm_seen < need + 8) { gm_pend = ld_u32_gpu(gmin_ptr); gm_inflight = true; }
+                        if (k > 0 && (int)gm_seen < need) {        // held back: work out the minimum itself, it may be stale
+                            gm_seen = poll_gmin(p.prog + (size_t)bl * p.NR * p.NC * CV_PROG_STRIDE, p.NR * p.NC,
+                                                p.gmin + (size_t)bl * CV_PROG_STRIDE, (unsigned)need, p.status);
+                            fresh = true;
+                        }
+                        if (fresh) {                               // acquire side, and generic -> async proxy (the TMA reads)
+                            __threadfence();
+                            asm volatile("fence.proxy.async.global;" ::: "memory");
+                        }
+                    }
                     if (k > 0) {
                         mbar_expect_tx(&sm.qbar[stp], (unsigned)(k * 8 * p.qp * 4));
                         tma_load_2d(sm.qs + (size_t)stp * (CV_PW * CV_PW), &p.qmap[k - 1], d.tma_col, d.tma_row, &sm.qbar[stp]);
@@ -726,16 +769,22 @@ conveyor_kernel(const __grid_constant__ CParams p)
         auto nbr_cta = [&](int which) {
             return (bl * p.NR + ((which & 2) ? ciu : ci)) * p.NC + ((which & 1) ? cjl : cj);
         };
+#if defined(SMRE_CV_EXP) && (SMRE_CV_EXP == 9 || SMRE_CV_EXP == 10)
+        unsigned long long *const box_l = p.mbox + (size_t)cta * CV_D * CV_MBW;
+        unsigned long long *const box_u = box_l, *const box_ul = box_l;
+#else
         unsigned long long *const box_l = p.mbox + (size_t)nbr_cta(1) * CV_D * CV_MBW;
         unsigned long long *const box_u = p.mbox + (size_t)nbr_cta(2) * CV_D * CV_MBW;
         unsigned long long *const box_ul = p.mbox + (size_t)nbr_cta(3) * CV_D * CV_MBW;
+#endif
         const unsigned *my_nbr_prog = p.prog + (size_t)nbr_cta(lane >= 1 && lane <= 3 ? lane : 1) * CV_PROG_STRIDE;
         unsigned prog_pend = 0, prog_seen = 0;  // lanes 1..3: progress of the receiving CTAs
         int prog_iter = -1;                     // step at which prog_pend was requested (-1: none in flight)
         // The sender warp of the first slot of a frame also keeps that frame's gmin: every few steps it reads all
         // progress counters of the frame (requested two steps before they are used) and publishes their minimum.
         const int tiles = p.NR * p.NC;
-        const bool keeper = tiles > 1 && ci == 0 && cj == 0;
+        const bool ordered = tiles > 1;
+        const bool keeper = ordered && ci == 0 && cj == 0;
         const unsigned *const frame_prog = p.prog + (size_t)bl * tiles * CV_PROG_STRIDE;
         unsigned *const gmin_out = p.gmin + (size_t)bl * CV_PROG_STRIDE;
         unsigned cnt[5] = {0, 0, 0, 0, 0};
@@ -743,7 +792,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
 #pragma unroll
             for (int k = 0; k < 5; ++k) {
                 const int i = lane + 32 * k;
-                cnt[k] = i < tiles ? ld_u32_gpu(frame_prog + (size_t)i * CV_PROG_STRIDE) : 0xffffffffu;
+                cnt[k] = i < tiles ? ld_u32_gpu(frame_prog + (size_t)i * CV_PROG_STRIDE + 1) : 0xffffffffu;
             }
         };
         auto publish_min = [&]() {
@@ -752,7 +801,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
             for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
             // atomicMax: this minimum may be older than one the receiver lane of this CTA has published while it
             // was held back; a bound that drops could hold back the very slot this one is waiting for
-            if (lane == 0) atomicMax(gmin_out, m);
+            if (lane == 0) { __threadfence(); atomicMax(gmin_out, m); }
             return m;
         };
         for (int g = 0; g < total; ++g) {
@@ -760,7 +809,11 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 if ((g & p.gmin_mask) == 0) read_counters();
                 else if ((g & p.gmin_mask) == 2) publish_min();
             }
+#if defined(SMRE_CV_EXP) && (SMRE_CV_EXP == 3 || SMRE_CV_EXP == 6)
+            if (false) {
+#else
             if (g > 0) {
+#endif
                 if ((g & 3) == 1 && lane >= 1 && lane <= 3) {
                     // Ring slots g .. g+4 (through the next check, so that helpers may send right away) must have
                     // been read by the receiver: its counter must have reached g + 4 - CV_D.  The counter is re-read only when the ring is half used, and the value is
@@ -774,7 +827,11 @@ conveyor_kernel(const __grid_constant__ CParams p)
                     }
                 }
                 __syncwarp();
+#if defined(SMRE_CV_EXP) && SMRE_CV_EXP == 10
+                const int slot = 0;
+#else
                 const int slot = (g % CV_D) * CV_MBW;
+#endif
                 const unsigned long long tag = (unsigned long long)(unsigned)g << 32;
                 // the first two departing lines of step g-1 (all there is except at changes of window edge)
                 const uint4 ln = *reinterpret_cast<const uint4 *>(&sm.desc[(g - 1) % CV_DR].send_a[0]);   // {a0, a1, b0, b1}
@@ -811,8 +868,19 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 }
                 // (lines beyond the second are sent by the compute warps: help_handoff)
             }
+            // Fenced progress (word 1 of the counter line; gmin is the minimum of these): the barrier of step g-1
+            // lies behind this warp, so the q writes of all steps <= g-1 have been issued; the fence makes them
+            // visible before the value g+1 is.  Every fence_mask + 1 steps only, after the sends: the fence takes ~1 us.
+            if (ordered && (g & p.fence_mask) == 1 && lane == 0) {
+                __threadfence();
+                st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE + 1, (unsigned)(g + 1));
+            }
             if (lane == 0) CV_STAMP(4);
             CV_STEP_BARRIER();
+        }
+        if (ordered && lane == 0) {                      // all steps done
+            __threadfence();
+            st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE + 1, (unsigned)(total + 1));
         }
         if (keeper) {
             // slower slots still need gmin: keep it until every counter has its final value (total - 1)
@@ -829,19 +897,6 @@ conveyor_kernel(const __grid_constant__ CParams p)
         // The first line (two chunks) of every step -- all there is in the usual step -- is located and
         // requested one step ahead; its geometry is kept in registers for the deposit a step later.
         unsigned long long *const my_box = p.mbox + (size_t)cta * CV_D * CV_MBW;
-        // The q of a pixel is written by one slot and read, a sweep (F steps) later, by a slot up / left of it,
-        // which orders the box CV_PF steps ahead of its use.  Hand-offs alone do not order the two: a boundary that
-        // does not move for some steps carries no message, and a slot without a tile waits for nothing.  So no
-        // slot runs more than `lead` = F - CV_PF - 3 steps ahead of gmin, a lower bound of every counter of
-        // the frame: the box of step g is ordered in iteration g - CV_PF, after the check of iteration
-        // g - CV_PF - 1, when every counter was >= g - CV_PF - 1 - lead = g - F + 2, i.e. every slot had issued the
-        // q writes of step g - F (a counter value v is stored after the barrier of step v - 2).  The natural lag
-        // of the pipeline is far smaller than a sweep of the usual configurations, so the check is almost free:
-        // gmin is re-read (a step before the value is needed) only when the last value seen gets old.
-        const unsigned *const gmin_ptr = p.gmin + (size_t)bl * CV_PROG_STRIDE;
-        unsigned gm_seen = 0, gm_pend = 0;           // lane 2
-        bool gm_inflight = false;
-        const bool paced = p.NR * p.NC > 1;
         unsigned long long pend[4] = {0, 0, 0, 0};
         int pxi[4] = {0, 0, 0, 0}, pwd[4] = {0, 0, 0, 0}, pn = 0;
         bool pok[4] = {false, false, false, false};
@@ -857,15 +912,29 @@ conveyor_kernel(const __grid_constant__ CParams p)
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                     const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
+#if defined(SMRE_CV_EXP) && SMRE_CV_EXP == 1
+                    pok[2 * l + u] = false;
+#else
                     pok[2 * l + u] = pos < len;
+#endif
                     pwd[2 * l + u] = (int)((a & 0xffffu) | v);
                     pxi[2 * l + u] = (int)((a >> 16) | (v << sh));
+#if defined(SMRE_CV_EXP) && SMRE_CV_EXP == 1
+                    pend[2 * l + u] = 0;
+#else
                     pend[2 * l + u] = ld_u64_gpu(box2 + pwd[2 * l + u]);       // unconditional: nothing waits on it
+#endif
                 }
             }
         };
+#if !defined(SMRE_CV_EXP) || SMRE_CV_EXP < 2 || SMRE_CV_EXP == 5 || SMRE_CV_EXP == 8
         if (total > 1) locate(1);
+#endif
+#if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 4
+        long long rclk[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
         for (int g = 0; g < total; ++g) {
+            CV_RCLK(0);
             if (g + 1 < total) {
                 const unsigned long long *box = my_box + (size_t)((g + 1) % CV_D) * CV_MBW;
                 const unsigned tag = (unsigned)(g + 1);
@@ -877,27 +946,31 @@ conveyor_kernel(const __grid_constant__ CParams p)
                         sm.xs[pxi[u]] = __uint_as_float((unsigned)w);
                     }
                 // (lines beyond the second are received by the compute warps: help_handoff)
+                CV_RCLK(1);
                 __syncwarp();
+                CV_RCLK(2);
                 if (lane == 0) CV_STAMP(2);
-                if (paced) {                                   // q ordering: at most `lead` steps ahead of gmin
-                    if (lane == 2) {
-                        if (gm_inflight) { gm_seen = max(gm_seen, gm_pend); gm_inflight = false; }
-                        else if ((int)gm_seen + p.lead < g + 8) { gm_pend = ld_u32_gpu(gmin_ptr); gm_inflight = true; }
-                        if ((int)gm_seen + p.lead < g)        // held back: work out the minimum itself, it may be stale
-                            gm_seen = poll_gmin(p.prog + (size_t)bl * p.NR * p.NC * CV_PROG_STRIDE, p.NR * p.NC,
-                                                p.gmin + (size_t)bl * CV_PROG_STRIDE, (unsigned)(g - p.lead), p.status);
-                    }
-                    __syncwarp();
-                }
+                CV_RCLK(3);
                 if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // step g+1 has been read
+                CV_RCLK(4);
+#if !defined(SMRE_CV_EXP) || SMRE_CV_EXP < 2 || SMRE_CV_EXP == 5 || SMRE_CV_EXP == 8
                 if (g + 2 < total) locate(g + 2);
+#endif
             }
             if (lane == 0 && (g & 7) == 3) {
                 if (status_pend) sm.abort = 1;
                 status_pend = *(volatile int *)p.status;             // consumed 8 steps later
             }
             if (lane == 0) CV_STAMP(5);
+            CV_RCLK(5);
             CV_STEP_BARRIER();
+#if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 4
+            if (p.trace && lane == 0) {
+                const long long t_end = clock64();
+                for (int i = 1; i < 6; ++i) p.trace[((size_t)cta * total + g) * 8 + i] = (unsigned long long)(rclk[i] - rclk[0]);
+                p.trace[((size_t)cta * total + g) * 8] = (unsigned long long)(t_end - rclk[0]);
+            }
+#endif
         }
     }
 
@@ -924,6 +997,15 @@ static ConveyorKernel kernel_for(int Wq)
 }
 
 // ---- host side ----------------------------------------------------------------------------------
+
+// The fenced counters are refreshed every fence_mask + 1 steps (a fence costs ~1 us): at most a third of the lead
+// a sweep allows.  gmin is recomputed from them every gmin_mask + 1 steps.
+static int fence_mask_for(int F)
+{
+    int m = 63;
+    while (m > 3 && m + 2 > (F - CV_PF - 2) / 3) m >>= 1;
+    return m;
+}
 
 struct DeviceTables {             // boundary tables of one n_sweeps value, resident on the device
     int n_sweeps = 0;
@@ -1009,11 +1091,12 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
     char why[160];
     // the tiling is chosen on a short run; tables_for() re-plans (and re-verifies) each real length
     if (!conveyor_summary(H, W, fams, 3, capacity, &cs, why, sizeof why)) return nullptr;
-    // With several tiles a slot may lead the slowest slot by F - CV_PF - 3 steps (q ordering, see the receiver
-    // warp); the pipeline wants some slack per tile to hide the latency of a hand-off.
-    // The tile that feeds another is at least one step ahead of it, so the last tile leads the first by the
-    // length of the chain between them; a lead with no slack beyond that would run, but in lock step.
-    if (cs.tiles_y * cs.tiles_x > 1 && (int)fams.size() - CV_PF - 3 < cs.tiles_y + cs.tiles_x + 4) return nullptr;
+    // With several tiles a slot may lead the slowest slot by F - CV_PF - 2 steps minus the age of the fenced
+    // counters (q ordering, see the control warp).  The tile that feeds another is at least one step ahead of it,
+    // so the last tile leads the first by the length of the chain between them; a lead with no slack beyond that
+    // would run, but in lock step.
+    if (cs.tiles_y * cs.tiles_x > 1 &&
+        (int)fams.size() - CV_PF - 2 - (fence_mask_for((int)fams.size()) + 2) < cs.tiles_y + cs.tiles_x + 4) return nullptr;
 
     ConveyorPlan *pl = new ConveyorPlan;
     pl->H = H; pl->W = W; pl->Wq = (W + 3) & ~3; pl->B = B; pl->F = (int)fams.size();
@@ -1110,8 +1193,8 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
     p.y = y; p.x_out = x_out; p.q = pl->q; p.fams = pl->d_fams; p.taby = tabs->d_y; p.tabx = tabs->d_x;
     p.mbox = pl->d_mbox; p.prog = pl->d_prog; p.status = pl->d_status;
     p.F = pl->F; p.total = pl->F * n_sweeps; p.H = pl->H; p.W = pl->W; p.Wq = pl->Wq; p.B_total = pl->B;
-    p.NR = pl->NR; p.NC = pl->NC; p.qp = pl->qp; p.lead = pl->F - CV_PF - 3;
-    p.gmin_mask = p.lead >= 64 ? 15 : p.lead >= 32 ? 7 : 3;
+    p.NR = pl->NR; p.NC = pl->NC; p.qp = pl->qp; p.fence_mask = fence_mask_for(pl->F);
+    p.gmin_mask = std::min(p.fence_mask, 15);
     p.gmin = pl->d_prog + (size_t)pl->frames_per_launch * pl->NR * pl->NC * CV_PROG_STRIDE;
     memcpy(p.qmap, pl->qmap, sizeof p.qmap);
     const int tiles = pl->NR * pl->NC;
