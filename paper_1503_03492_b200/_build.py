@@ -29,8 +29,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
         cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
         if os.environ.get("SMRE_CV_TRACE_BUILD"):
             cmd.insert(1, "-DSMRE_CV_TRACE_BUILD=" + os.environ["SMRE_CV_TRACE_BUILD"])
-        if os.environ.get("SMRE_CV_EXP"):
-            cmd.insert(1, "-DSMRE_CV_EXP=" + os.environ["SMRE_CV_EXP"])
         if os.environ.get("SMRE_DEBUG"):
             cmd.insert(1, "-DSMRE_DEBUG")
         else:

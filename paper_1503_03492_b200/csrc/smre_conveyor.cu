@@ -73,17 +73,16 @@ __device__ __forceinline__ unsigned long long ld_u64_gpu(const unsigned long lon
     return v;
 }
 __device__ __forceinline__ void st_u64_gpu(unsigned long long *p, unsigned long long v) {
-#if defined(SMRE_CV_EXP) && SMRE_CV_EXP == 7
-    if (v == 0x123456789abcull) asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-#elif defined(SMRE_CV_EXP) && SMRE_CV_EXP == 8
-    asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-#else
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-#endif
 }
 __device__ __forceinline__ unsigned ld_u32_gpu(const unsigned *p) {
     unsigned v;
     asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned ld_acquire_u32_gpu(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void st_u32_gpu(unsigned *p, unsigned v) {
@@ -568,9 +567,6 @@ __device__ __forceinline__ int arrival_chunks(const AxisEntry &Y, const AxisEntr
 // (line 2 + warp, + CV_NCW, ...) during the step in which they are due.
 __device__ __noinline__ void help_handoff(Smem &sm, const CParams &p, int g, unsigned help, int warp, int lane)
 {
-#if defined(SMRE_CV_EXP) && (SMRE_CV_EXP == 3 || SMRE_CV_EXP == 5 || SMRE_CV_EXP == 7 || SMRE_CV_EXP == 9 || SMRE_CV_EXP == 10)
-    return;
-#endif
     const int cta = blockIdx.x;
     const int bl = cta / (p.NR * p.NC);
     const int t2 = cta - bl * p.NR * p.NC;
@@ -731,14 +727,17 @@ conveyor_kernel(const __grid_constant__ CParams p)
                     if (ordered) {
                         const int need = g + CV_PF - p.F + 2;
                         bool fresh = false;
-                        if (gm_inflight) { gm_seen = max(gm_seen, gm_pend); gm_inflight = false; fresh = true; }
-                        else if ((int)gm_seen < need + 8) { gm_pend = ld_u32_gpu(gmin_ptr); gm_inflight = true; }
+                        if (gm_inflight) {
+                            gm_seen = max(gm_seen, gm_pend); gm_inflight = false;
+                            asm volatile("fence.proxy.async.global;" ::: "memory");     // generic -> async proxy (the TMA reads)
+                        }
+                        else if ((int)gm_seen < need + 8) { gm_pend = ld_acquire_u32_gpu(gmin_ptr); gm_inflight = true; }
                         if (k > 0 && (int)gm_seen < need) {        // held back: work out the minimum itself, it may be stale
                             gm_seen = poll_gmin(p.prog + (size_t)bl * p.NR * p.NC * CV_PROG_STRIDE, p.NR * p.NC,
                                                 p.gmin + (size_t)bl * CV_PROG_STRIDE, (unsigned)need, p.status);
                             fresh = true;
                         }
-                        if (fresh) {                               // acquire side, and generic -> async proxy (the TMA reads)
+                        if (fresh) {                               // (rare) acquire side, and generic -> async proxy
                             __threadfence();
                             asm volatile("fence.proxy.async.global;" ::: "memory");
                         }
@@ -769,14 +768,9 @@ conveyor_kernel(const __grid_constant__ CParams p)
         auto nbr_cta = [&](int which) {
             return (bl * p.NR + ((which & 2) ? ciu : ci)) * p.NC + ((which & 1) ? cjl : cj);
         };
-#if defined(SMRE_CV_EXP) && (SMRE_CV_EXP == 9 || SMRE_CV_EXP == 10)
-        unsigned long long *const box_l = p.mbox + (size_t)cta * CV_D * CV_MBW;
-        unsigned long long *const box_u = box_l, *const box_ul = box_l;
-#else
         unsigned long long *const box_l = p.mbox + (size_t)nbr_cta(1) * CV_D * CV_MBW;
         unsigned long long *const box_u = p.mbox + (size_t)nbr_cta(2) * CV_D * CV_MBW;
         unsigned long long *const box_ul = p.mbox + (size_t)nbr_cta(3) * CV_D * CV_MBW;
-#endif
         const unsigned *my_nbr_prog = p.prog + (size_t)nbr_cta(lane >= 1 && lane <= 3 ? lane : 1) * CV_PROG_STRIDE;
         unsigned prog_pend = 0, prog_seen = 0;  // lanes 1..3: progress of the receiving CTAs
         int prog_iter = -1;                     // step at which prog_pend was requested (-1: none in flight)
@@ -805,15 +799,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
             return m;
         };
         for (int g = 0; g < total; ++g) {
-            if (keeper) {
-                if ((g & p.gmin_mask) == 0) read_counters();
-                else if ((g & p.gmin_mask) == 2) publish_min();
-            }
-#if defined(SMRE_CV_EXP) && (SMRE_CV_EXP == 3 || SMRE_CV_EXP == 6)
-            if (false) {
-#else
             if (g > 0) {
-#endif
                 if ((g & 3) == 1 && lane >= 1 && lane <= 3) {
                     // Ring slots g .. g+4 (through the next check, so that helpers may send right away) must have
                     // been read by the receiver: its counter must have reached g + 4 - CV_D.  The counter is re-read only when the ring is half used, and the value is
@@ -827,11 +813,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
                     }
                 }
                 __syncwarp();
-#if defined(SMRE_CV_EXP) && SMRE_CV_EXP == 10
-                const int slot = 0;
-#else
                 const int slot = (g % CV_D) * CV_MBW;
-#endif
                 const unsigned long long tag = (unsigned long long)(unsigned)g << 32;
                 // the first two departing lines of step g-1 (all there is except at changes of window edge)
                 const uint4 ln = *reinterpret_cast<const uint4 *>(&sm.desc[(g - 1) % CV_DR].send_a[0]);   // {a0, a1, b0, b1}
@@ -875,6 +857,10 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 __threadfence();
                 st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE + 1, (unsigned)(g + 1));
             }
+            if (keeper) {                                  // (after the sends as well: publishing fences too)
+                if ((g & p.gmin_mask) == 0) read_counters();
+                else if ((g & p.gmin_mask) == 2) publish_min();
+            }
             if (lane == 0) CV_STAMP(4);
             CV_STEP_BARRIER();
         }
@@ -912,24 +898,14 @@ conveyor_kernel(const __grid_constant__ CParams p)
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                     const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
-#if defined(SMRE_CV_EXP) && SMRE_CV_EXP == 1
-                    pok[2 * l + u] = false;
-#else
                     pok[2 * l + u] = pos < len;
-#endif
                     pwd[2 * l + u] = (int)((a & 0xffffu) | v);
                     pxi[2 * l + u] = (int)((a >> 16) | (v << sh));
-#if defined(SMRE_CV_EXP) && SMRE_CV_EXP == 1
-                    pend[2 * l + u] = 0;
-#else
                     pend[2 * l + u] = ld_u64_gpu(box2 + pwd[2 * l + u]);       // unconditional: nothing waits on it
-#endif
                 }
             }
         };
-#if !defined(SMRE_CV_EXP) || SMRE_CV_EXP < 2 || SMRE_CV_EXP == 5 || SMRE_CV_EXP == 8
         if (total > 1) locate(1);
-#endif
 #if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 4
         long long rclk[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
@@ -953,9 +929,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 CV_RCLK(3);
                 if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // step g+1 has been read
                 CV_RCLK(4);
-#if !defined(SMRE_CV_EXP) || SMRE_CV_EXP < 2 || SMRE_CV_EXP == 5 || SMRE_CV_EXP == 8
                 if (g + 2 < total) locate(g + 2);
-#endif
             }
             if (lane == 0 && (g & 7) == 3) {
                 if (status_pend) sm.abort = 1;
