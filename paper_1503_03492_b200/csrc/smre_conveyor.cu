@@ -209,13 +209,15 @@ struct Smem {
     unsigned long long qbar[CV_NST];         // mbarriers: the TMA box of a stage has landed
     CFamily fams[CV_MAX_F];
     int abort;                               // set by the receiver warp when the failure flag is up
+    int cur_step;                            // control warp -> planner warp: the step the CTA is in
+    int planned;                             // planner warp -> control warp: steps [0, planned) have descriptors
 };
 
 // One barrier per step.  Every 8th step all warps also look at Smem::abort (set only at steps = 3 mod 8,
 // so that every warp reads the same value) and leave together if a hand-off has timed out somewhere.
 #define CV_STEP_BARRIER()                                                         \
     do {                                                                          \
-        __syncthreads();                                                          \
+        asm volatile("bar.sync 1, %0;" ::"n"(CV_NST_T) : "memory");              \
         if ((g & 7) == 7 && *(volatile int *)&sm.abort) return;                   \
     } while (0)
 
@@ -644,11 +646,11 @@ conveyor_kernel(const __grid_constant__ CParams p)
 
     // ---- prologue: families and the first table entries into shared memory; x <- y on the tile ----
     for (int i = tid; i < p.F; i += CV_NT) sm.fams[i] = p.fams[i];
-    for (int i = tid; i < 2 * min(total, 2 * CV_BATCH); i += CV_NT) {
+    for (int i = tid; i < 2 * min(total, 3 * CV_BATCH); i += CV_NT) {
         const int g = i >> 1, ax = i & 1;
         sm.tab[g % CV_TR][ax] = ax ? p.tabx[(size_t)g * p.NC + cj] : p.taby[(size_t)g * p.NR + ci];
     }
-    if (tid == 0) sm.abort = 0;
+    if (tid == 0) { sm.abort = 0; sm.cur_step = 0; sm.planned = CV_AHEAD; }
     __syncthreads();
     {
         const AxisEntry ey = sm.tab[0][0], ex = sm.tab[0][1];
@@ -666,8 +668,8 @@ conveyor_kernel(const __grid_constant__ CParams p)
             for (int i = 0; i < CV_NST; ++i) mbar_init(&sm.qbar[i], 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
-        plan_steps(sm, p, 0, CV_AHEAD, lane, total, frame_off_q, plane, p.frame0 + bl, geom, key);
     }
+    if (warp == CV_NCW + 3) plan_steps(sm, p, 0, CV_AHEAD, lane, total, frame_off_q, plane, p.frame0 + bl, geom, key);
     __syncthreads();
 
     if (warp < CV_NCW) {
@@ -712,15 +714,23 @@ conveyor_kernel(const __grid_constant__ CParams p)
         bool gm_inflight = false;
         const bool ordered = p.NR * p.NC > 1;
         for (int g = 0; g < total; ++g) {
-            if ((g & (CV_BATCH - 1)) == 0) {
-                // table entries of steps [g + 32, g + 48); those fetched 16 steps ago are complete and visible
-                cp_async_wait<0>();
-                __syncwarp();
-                fetch_table(sm, p, g + 2 * CV_BATCH, lane, ci, cj, total);
-                plan_steps(sm, p, g + CV_AHEAD, CV_BATCH, lane, total, frame_off_q, plane, p.frame0 + bl, geom, key);
-                __syncwarp();
-            }
             if (lane == 0) {
+                // (release at CTA scope: the services warp fences the q writes of the steps before this one)
+                __threadfence_block();
+                *(volatile int *)&sm.cur_step = g;                   // paces the services warp
+                constexpr int CK = CV_BATCH - 1 - CV_PF < CV_BATCH / 2 ? CV_BATCH - 1 - CV_PF : CV_BATCH / 2;
+                static_assert(CK >= 2, "the services warp needs a few steps for a batch of descriptors");
+                if ((g & (CV_BATCH - 1)) == CK) {
+                    // The descriptors of steps [g - CK + 16, g - CK + 32) were released to the services warp at step
+                    // g - CK; nobody has looked beyond step g - 1 + CV_PF < g - CK + 16 so far.  Normally they are long done.
+                    const int need = min(total, g - CK + CV_AHEAD + CV_BATCH);
+                    const long long t0 = clock64();
+                    while (*(volatile int *)&sm.planned < need) {
+                        if (*(volatile int *)&sm.abort) break;
+                        if (clock64() - t0 > 2000000000LL) { atomicExch(p.status, 1); break; }
+                    }
+                    __threadfence_block();
+                }
                 if (g + CV_PF < total) {                             // order the q box of step g + CV_PF
                     const StepDesc &d = sm.desc[(g + CV_PF) % CV_DR];
                     const int k = d.tma_k;
@@ -761,6 +771,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
             if (++st1 == CV_NST) st1 = 0;
             if (++stp == CV_NST) stp = 0;
         }
+        if (lane == 0) { __threadfence_block(); *(volatile int *)&sm.cur_step = total; }   // all steps done
     } else if (warp == CV_NCW + 1) {
         // =============== sender warp: departures of step g-1 -> the neighbours' mailboxes, tagged g ======
         // receivers of departing pixels: bit 0 = left neighbour, bit 1 = upper neighbour (3 = up-left)
@@ -774,30 +785,6 @@ conveyor_kernel(const __grid_constant__ CParams p)
         const unsigned *my_nbr_prog = p.prog + (size_t)nbr_cta(lane >= 1 && lane <= 3 ? lane : 1) * CV_PROG_STRIDE;
         unsigned prog_pend = 0, prog_seen = 0;  // lanes 1..3: progress of the receiving CTAs
         int prog_iter = -1;                     // step at which prog_pend was requested (-1: none in flight)
-        // The sender warp of the first slot of a frame also keeps that frame's gmin: every few steps it reads all
-        // progress counters of the frame (requested two steps before they are used) and publishes their minimum.
-        const int tiles = p.NR * p.NC;
-        const bool ordered = tiles > 1;
-        const bool keeper = ordered && ci == 0 && cj == 0;
-        const unsigned *const frame_prog = p.prog + (size_t)bl * tiles * CV_PROG_STRIDE;
-        unsigned *const gmin_out = p.gmin + (size_t)bl * CV_PROG_STRIDE;
-        unsigned cnt[5] = {0, 0, 0, 0, 0};
-        auto read_counters = [&]() {
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                const int i = lane + 32 * k;
-                cnt[k] = i < tiles ? ld_u32_gpu(frame_prog + (size_t)i * CV_PROG_STRIDE + 1) : 0xffffffffu;
-            }
-        };
-        auto publish_min = [&]() {
-            unsigned m = min(min(min(cnt[0], cnt[1]), min(cnt[2], cnt[3])), cnt[4]);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
-            // atomicMax: this minimum may be older than one the receiver lane of this CTA has published while it
-            // was held back; a bound that drops could hold back the very slot this one is waiting for
-            if (lane == 0) { __threadfence(); atomicMax(gmin_out, m); }
-            return m;
-        };
         for (int g = 0; g < total; ++g) {
             if (g > 0) {
                 if ((g & 3) == 1 && lane >= 1 && lane <= 3) {
@@ -850,26 +837,85 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 }
                 // (lines beyond the second are sent by the compute warps: help_handoff)
             }
-            // Fenced progress (word 1 of the counter line; gmin is the minimum of these): the barrier of step g-1
-            // lies behind this warp, so the q writes of all steps <= g-1 have been issued; the fence makes them
-            // visible before the value g+1 is.  Every fence_mask + 1 steps only, after the sends: the fence takes ~1 us.
-            if (ordered && (g & p.fence_mask) == 1 && lane == 0) {
-                __threadfence();
-                st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE + 1, (unsigned)(g + 1));
-            }
-            if (keeper) {                                  // (after the sends as well: publishing fences too)
-                if ((g & p.gmin_mask) == 0) read_counters();
-                else if ((g & p.gmin_mask) == 2) publish_min();
-            }
             if (lane == 0) CV_STAMP(4);
             CV_STEP_BARRIER();
         }
-        if (ordered && lane == 0) {                      // all steps done
-            __threadfence();
-            st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE + 1, (unsigned)(total + 1));
+    } else if (warp == CV_NCW + 3) {
+        // =============== services warp: everything that is slow and that nobody has to wait for ===================
+        // Paced by Smem::cur_step only; it never joins the step barrier.  (a) Descriptors of steps [16 b + 16,
+        // 16 b + 32) as soon as step 16 b runs (~2-3 us per batch; rings: a batch overwrites descriptors of steps
+        // < 16 b - 32 and table entries of steps < 16 b - 64, all retired by then).  (b) The mailbox progress counter
+        // (word 0): when the CTA is in step c, its receiver has read the arrivals of step c.  (c) The fenced counter
+        // (word 1; gmin is the minimum of these): the barrier of step c - 1 lies behind the CTA, so the q writes of all
+        // steps <= c - 1 have been issued; control's CTA-scope release of cur_step and this warp's fence make them
+        // visible before the value c + 1 is.  Every fence_mask + 1 steps (a fence takes 1-4 us).  (d) The first slot
+        // of a frame keeps that frame's gmin.
+        const int tiles = p.NR * p.NC;
+        const bool ordered = tiles > 1;
+        const bool keeper = ordered && ci == 0 && cj == 0;
+        const unsigned *const frame_prog = p.prog + (size_t)bl * tiles * CV_PROG_STRIDE;
+        unsigned *const gmin_out = p.gmin + (size_t)bl * CV_PROG_STRIDE;
+        unsigned cnt[5] = {0, 0, 0, 0, 0};
+        auto read_counters = [&]() {
+#pragma unroll
+            for (int k = 0; k < 5; ++k) {
+                const int i = lane + 32 * k;
+                cnt[k] = i < tiles ? ld_u32_gpu(frame_prog + (size_t)i * CV_PROG_STRIDE + 1) : 0xffffffffu;
+            }
+        };
+        auto publish_min = [&]() {
+            unsigned m = min(min(min(cnt[0], cnt[1]), min(cnt[2], cnt[3])), cnt[4]);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
+            // atomicMax: this minimum may be older than one the receiver lane of this CTA has published while it
+            // was held back; a bound that drops could hold back the very slot this one is waiting for
+            if (lane == 0) { __threadfence(); atomicMax(gmin_out, m); }
+            return m;
+        };
+        int next_b = 0, seen = -1, last_fence = -1000000, last_keep = -1000000;
+        long long t_last = clock64();
+        bool dead = false;
+        for (;;) {
+            int c = 0;
+            if (lane == 0) c = *(volatile int *)&sm.cur_step;
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c == seen) {
+                int bad = 0;
+                if (lane == 0) bad = *(volatile int *)&sm.abort || clock64() - t_last > 4000000000LL;
+                if (__shfl_sync(0xffffffffu, bad, 0)) { dead = true; break; }
+                __nanosleep(40);
+                continue;
+            }
+            seen = c;
+            t_last = clock64();
+            const bool fin = c >= total;
+            if (lane == 0) {
+                __threadfence_block();                               // acquire side of cur_step (CTA scope)
+                st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)min(c, total - 1));
+            }
+            if (ordered && (fin || c - last_fence > p.fence_mask)) {
+                last_fence = c;
+                if (lane == 0) {
+                    __threadfence();
+                    st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE + 1, (unsigned)(c + 1));
+                }
+            }
+            if (keeper && (fin || c - last_keep > p.gmin_mask)) { last_keep = c; read_counters(); publish_min(); }
+            if (fin) break;
+            if (CV_BATCH * next_b + CV_AHEAD < total && c >= CV_BATCH * next_b) {
+                cp_async_wait<0>();                                  // table entries fetched a batch ago
+                __syncwarp();
+                fetch_table(sm, p, CV_BATCH * next_b + 3 * CV_BATCH, lane, ci, cj, total);
+                plan_steps(sm, p, CV_BATCH * next_b + CV_AHEAD, CV_BATCH, lane, total, frame_off_q, plane, p.frame0 + bl, geom, key);
+                __threadfence_block();
+                __syncwarp();
+                if (lane == 0) *(volatile int *)&sm.planned = CV_BATCH * next_b + CV_AHEAD + CV_BATCH;
+                ++next_b;
+            }
         }
-        if (keeper) {
-            // slower slots still need gmin: keep it until every counter has its final value (total - 1)
+        cp_async_wait<0>();
+        if (keeper && !dead) {
+            // slower slots still need gmin: keep it until every counter has its final value (total + 1)
             const long long t0 = clock64();
             for (;;) {
                 read_counters();
@@ -880,17 +926,17 @@ conveyor_kernel(const __grid_constant__ CParams p)
         }
     } else {
         // =============== receiver warp: arrivals of step g+1 into the tile ================================
-        // The first line (two chunks) of every step -- all there is in the usual step -- is located and
-        // requested one step ahead; its geometry is kept in registers for the deposit a step later.
+        // The first two lines (two chunks each) of every step -- all there is in the usual step -- are located and
+        // requested one step ahead, right after the deposit of the previous set; their geometry is kept in
+        // registers.  (Requesting them earlier -- at the start of that step -- was measured: 42.5 ms against 38.8 ms
+        // on C1.  The feeding tile is usually only just ahead, an early request misses its tag and pays a poll.)
         unsigned long long *const my_box = p.mbox + (size_t)cta * CV_D * CV_MBW;
-        unsigned long long pend[4] = {0, 0, 0, 0};
-        int pxi[4] = {0, 0, 0, 0}, pwd[4] = {0, 0, 0, 0}, pn = 0;
-        bool pok[4] = {false, false, false, false};
+        struct Pending { unsigned long long w[4]; int xi[4], wd[4]; bool ok[4]; };
+        Pending pc{};
         int status_pend = 0;                         // lane 0: the failure flag, loaded a step ahead
-        auto locate = [&](int step) {                // chunks 0..3 of `step` from the planner; requests their words
+        auto locate = [&](int step, Pending &q) {    // chunks 0..3 of `step` from the planner; requests their words
             const uint4 ln = *reinterpret_cast<const uint4 *>(&sm.desc[step % CV_DR].recv_a[0]);   // {a0, a1, b0, b1}
             const unsigned long long *box2 = my_box + (size_t)(step % CV_D) * CV_MBW;
-            pn = (int)(ln.z >> 24);
 #pragma unroll
             for (int l = 0; l < 2; ++l) {
                 const unsigned a = l ? ln.y : ln.x, b = l ? ln.w : ln.z;
@@ -898,14 +944,14 @@ conveyor_kernel(const __grid_constant__ CParams p)
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                     const unsigned pos = (u << 5) + lane, v = (var0 + pos) & 63u;
-                    pok[2 * l + u] = pos < len;
-                    pwd[2 * l + u] = (int)((a & 0xffffu) | v);
-                    pxi[2 * l + u] = (int)((a >> 16) | (v << sh));
-                    pend[2 * l + u] = ld_u64_gpu(box2 + pwd[2 * l + u]);       // unconditional: nothing waits on it
+                    q.ok[2 * l + u] = pos < len;
+                    q.wd[2 * l + u] = (int)((a & 0xffffu) | v);
+                    q.xi[2 * l + u] = (int)((a >> 16) | (v << sh));
+                    q.w[2 * l + u] = ld_u64_gpu(box2 + q.wd[2 * l + u]);       // unconditional: nothing waits on it
                 }
             }
         };
-        if (total > 1) locate(1);
+        if (total > 1) locate(1, pc);
 #if defined(SMRE_CV_TRACE_BUILD) && SMRE_CV_TRACE_BUILD == 4
         long long rclk[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
@@ -916,10 +962,10 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 const unsigned tag = (unsigned)(g + 1);
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                    if (pok[u]) {
-                        unsigned long long w = pend[u];
-                        if ((unsigned)(w >> 32) != tag) w = poll_tag(box + pwd[u], tag, p.status);
-                        sm.xs[pxi[u]] = __uint_as_float((unsigned)w);
+                    if (pc.ok[u]) {
+                        unsigned long long w = pc.w[u];
+                        if ((unsigned)(w >> 32) != tag) w = poll_tag(box + pc.wd[u], tag, p.status);
+                        sm.xs[pc.xi[u]] = __uint_as_float((unsigned)w);
                     }
                 // (lines beyond the second are received by the compute warps: help_handoff)
                 CV_RCLK(1);
@@ -927,9 +973,9 @@ conveyor_kernel(const __grid_constant__ CParams p)
                 CV_RCLK(2);
                 if (lane == 0) CV_STAMP(2);
                 CV_RCLK(3);
-                if (lane == 0) st_u32_gpu(p.prog + (size_t)cta * CV_PROG_STRIDE, (unsigned)(g + 1));   // step g+1 has been read
+                // (the services warp publishes "step g+1 has been read" when it sees the CTA in step g+1)
                 CV_RCLK(4);
-                if (g + 2 < total) locate(g + 2);
+                if (g + 2 < total) locate(g + 2, pc);
             }
             if (lane == 0 && (g & 7) == 3) {
                 if (status_pend) sm.abort = 1;
@@ -949,6 +995,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
     }
 
     // ---- a9: x_out <- the tile of the last step -----------------------------------------------------
+    __syncthreads();                                             // the planner warp joins the others here
     {
         const AxisEntry ey = sm.tab[(total - 1) % CV_TR][0], ex = sm.tab[(total - 1) % CV_TR][1];
         const int h = ey.R - ey.L, w = ex.R - ex.L;
@@ -974,10 +1021,11 @@ static ConveyorKernel kernel_for(int Wq)
 
 // The fenced counters are refreshed every fence_mask + 1 steps (a fence costs ~1 us): at most a third of the lead
 // a sweep allows.  gmin is recomputed from them every gmin_mask + 1 steps.
+constexpr int CV_SVC_LAG = 4;      // steps the services warp may be late with a counter (it also plans: 2-3 us per batch)
 static int fence_mask_for(int F)
 {
     int m = 63;
-    while (m > 3 && m + 2 > (F - CV_PF - 2) / 3) m >>= 1;
+    while (m > 3 && m + 2 + CV_SVC_LAG > (F - CV_PF - 2) / 3) m >>= 1;
     return m;
 }
 
@@ -1070,7 +1118,7 @@ ConveyorPlan *conveyor_plan_create(int H, int W, int B, const std::vector<Family
     // so the last tile leads the first by the length of the chain between them; a lead with no slack beyond that
     // would run, but in lock step.
     if (cs.tiles_y * cs.tiles_x > 1 &&
-        (int)fams.size() - CV_PF - 2 - (fence_mask_for((int)fams.size()) + 2) < cs.tiles_y + cs.tiles_x + 4) return nullptr;
+        (int)fams.size() - CV_PF - 2 - (fence_mask_for((int)fams.size()) + 2 + CV_SVC_LAG) < cs.tiles_y + cs.tiles_x + 4) return nullptr;
 
     ConveyorPlan *pl = new ConveyorPlan;
     pl->H = H; pl->W = W; pl->Wq = (W + 3) & ~3; pl->B = B; pl->F = (int)fams.size();

@@ -10,16 +10,17 @@
 namespace smre {
 
 constexpr int CV_NCW = 16;              // compute warps per CTA
-constexpr int CV_NT = (CV_NCW + 3) * 32;    // + one control, one sender, one receiver warp
+constexpr int CV_NST_T = (CV_NCW + 3) * 32;  // threads that take part in the step barrier: + one control, one sender, one receiver warp
+constexpr int CV_NT = CV_NST_T + 32;        // + the planner warp, which runs ahead of the steps and never joins their barrier
 constexpr int CV_PW = 64;               // edge of the torus-addressed x tile in shared memory
 constexpr int CV_SD = 16;               // strip depth: a boundary moves < CV_SD pixels per step
 constexpr int CV_D = 16;                // mailbox ring depth (steps)
-constexpr int CV_PF = 5;                // q prefetch distance (steps)
+constexpr int CV_PF = 7;                // q prefetch distance (steps)
 constexpr int CV_NST = CV_PF + 1;       // q stages in shared memory
-constexpr int CV_TR = 64;               // table ring entries in shared memory (steps)
-constexpr int CV_DR = 32;               // step descriptor ring (steps)
-constexpr int CV_BATCH = 16;            // the control warp plans this many steps at once, one per lane
-constexpr int CV_AHEAD = 8;             // ... starting this many steps ahead of the step it runs in
+constexpr int CV_TR = 128;              // table ring entries in shared memory (steps)
+constexpr int CV_DR = 64;               // step descriptor ring (steps)
+constexpr int CV_BATCH = 16;            // the planner warp plans this many steps at once, one per lane
+constexpr int CV_AHEAD = 16;            // ... starting this many steps ahead of the step that releases the batch
 constexpr int CV_MBW = 2 * CV_SD * CV_PW;   // 8-byte words per mailbox slot
 constexpr int CV_PROG_STRIDE = 64;       // progress counters 256 bytes apart: no line is shared by two CTAs
 constexpr int CV_MAX_F = 1024;          // families kept in shared memory
