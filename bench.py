@@ -231,8 +231,8 @@ def run_gpu(args, w, rank, world):
         if w.variant == "standard" and launch[0] == smre.SMRE_SCHED_PERSISTENT and w.name.startswith("C1") \
                 and w.n_sweeps == 200:
             # dram__bytes_read.sum + dram__bytes_write.sum of this launch from the committed ncu --set full
-            # capture (profiles/r01_ncu_full_conveyor_c1_metrics.txt): 39.668 GB + 41.152 GB
-            roofline["traffic"] = 80.820e9
+            # capture (profiles/r01_ncu_full_conveyor_c1_metrics.txt): 41.626 GB + 42.328 GB
+            roofline["traffic"] = 83.954e9
             roofline["traffic_source"] = "profiles/r01_ncu_full_conveyor_c1_metrics.txt"
         if w.variant != "standard":
             # ICD keeps q in registers: it is bound by fp32 issue, not by HBM.  Model: 5 fp32
