@@ -108,10 +108,10 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned long long *bar, unsigned 
                  : "=r"(ok) : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ void tma_load_2d(void *smem_dst, const CUtensorMap *map, int c0, int c1, unsigned long long *bar) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+__device__ __forceinline__ void tma_load_2d_hint(void *smem_dst, const CUtensorMap *map, int c0, int c1, unsigned long long *bar, unsigned long long pol) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;"
                  ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(map), "r"(c0), "r"(c1),
-                   "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+                   "r"((unsigned)__cvta_generic_to_shared(bar)), "l"(pol) : "memory");
 }
 
 // Spin until the mailbox word carries `tag`.  A poll that outlives ~1 s (or sees another CTA's failure)
@@ -710,6 +710,8 @@ conveyor_kernel(const __grid_constant__ CParams p)
         // head) is far smaller than a sweep of the usual configurations, and gmin is re-read, a step before the
         // value is needed, only when the last value seen gets old: the check is almost free.
         const unsigned *const gmin_ptr = p.gmin + (size_t)bl * CV_PROG_STRIDE;
+        unsigned long long q_policy = 0;       // q is read once per sweep: its lines should leave L2 first
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(q_policy));
         unsigned gm_seen = 0, gm_pend = 0;     // lane 0
         bool gm_inflight = false;
         const bool ordered = p.NR * p.NC > 1;
@@ -754,7 +756,7 @@ conveyor_kernel(const __grid_constant__ CParams p)
                     }
                     if (k > 0) {
                         mbar_expect_tx(&sm.qbar[stp], (unsigned)(k * 8 * p.qp * 4));
-                        tma_load_2d(sm.qs + (size_t)stp * (CV_PW * CV_PW), &p.qmap[k - 1], d.tma_col, d.tma_row, &sm.qbar[stp]);
+                        tma_load_2d_hint(sm.qs + (size_t)stp * (CV_PW * CV_PW), &p.qmap[k - 1], d.tma_col, d.tma_row, &sm.qbar[stp], q_policy);
                     }
                 }
                 CV_STAMP(7);
