@@ -149,7 +149,8 @@ def run_gpu(args, w, rank, world):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     sched = {"auto": smre.SMRE_SCHED_AUTO, "graph": smre.SMRE_SCHED_GRAPH,
-             "persistent": smre.SMRE_SCHED_PERSISTENT, "conveyor": smre.SMRE_SCHED_PERSISTENT}[args.schedule]
+             "persistent": smre.SMRE_SCHED_PERSISTENT, "conveyor": smre.SMRE_SCHED_PERSISTENT,
+             "strips": smre.SMRE_SCHED_STRIPS}[args.schedule]
     nums = workload_numbers(w)
     sol = smre.Solver(w.H, w.W, w.sides, w.c, w.variant, w.batch, sched)
     stream = torch.cuda.Stream()
@@ -259,7 +260,7 @@ def run_gpu(args, w, rank, world):
             "config": {"workload": w.name, "note": w.note, "variant": w.variant, "n_sweeps": w.n_sweeps,
                        "H": w.H, "W": w.W, "batch": w.batch, "families": nums["families"],
                        "windows_per_sweep": nums["windows_per_sweep"],
-                       "schedule": ("icd_shifts" if w.variant != "standard" else {1: "graph", 2: "conveyor"}.get(launch[0], str(launch[0]))),
+                       "schedule": ("icd_shifts" if w.variant != "standard" else {1: "graph", 2: "conveyor", 3: "strips"}.get(launch[0], str(launch[0]))),
                        "tiles": [launch[2], launch[3]],
                        "l2": ("q planes (204 MiB for C1, > 126 MB L2) are rewritten by every step: nothing of a step survives "
                               "in L2 for the next one") if flush is None else "256 MiB flush between steps",
@@ -286,7 +287,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1)")
     ap.add_argument("--n-sweeps", type=int, default=None, help="override the config's sweep count (debug)")
-    ap.add_argument("--schedule", default="auto", choices=["auto", "graph", "persistent", "conveyor"])
+    ap.add_argument("--schedule", default="auto", choices=["auto", "graph", "persistent", "conveyor", "strips"])
     ap.add_argument("--ref-sweeps", type=int, default=200, help="oracle sample size in sweeps (~12 s on C1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -56,9 +56,10 @@ typedef enum { SMRE_STANDARD = 0, SMRE_INCOMPLETE = 1 } smre_variant;
 typedef enum {
     SMRE_SCHED_AUTO = 0,        /* persistent if the image tiles fit on chip, else graph */
     SMRE_SCHED_GRAPH = 1,       /* one kernel per family, one captured CUDA graph per sweep */
-    SMRE_SCHED_PERSISTENT = 2   /* "conveyor": one cooperative kernel per call; x tiles resident in
+    SMRE_SCHED_PERSISTENT = 2,  /* "conveyor": one cooperative kernel per call; x tiles resident in
                                    shared memory, tile boundaries that follow each family's window
                                    grid, one-directional hand-off between CTAs, q streamed from HBM */
+    SMRE_SCHED_STRIPS = 3       /* one cooperative kernel per call; one CTA per strip of 8 rows */
 } smre_schedule;
 
 #define SMRE_MAX_SIDE 32        /* largest window side (the paper's L_SMRE = 32) */

@@ -4,7 +4,7 @@ Thin Python binding over the C ABI of include/smre.h (argument marshalling only;
 supplies device memory and streams).  Shares nothing with the test oracle.
 """
 from .smre import (  # noqa: F401
-    SMRE_INCOMPLETE, SMRE_SCHED_AUTO, SMRE_SCHED_GRAPH, SMRE_SCHED_PERSISTENT, SMRE_STANDARD,
+    SMRE_INCOMPLETE, SMRE_SCHED_AUTO, SMRE_SCHED_GRAPH, SMRE_SCHED_PERSISTENT, SMRE_SCHED_STRIPS, SMRE_STANDARD,
     SmreError, Solver, exported_symbols, lib_path, load_library, smre_create, smre_destroy,
     smre_export_increments, smre_family, smre_info, smre_last_error, smre_last_launch,
     smre_plan_check, smre_project, smre_project_host, smre_set_schedule,

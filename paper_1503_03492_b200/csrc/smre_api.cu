@@ -4,6 +4,7 @@
 #include "../../include/smre.h"
 #include "smre_common.cuh"
 #include "smre_conveyor.cuh"
+#include "smre_strips.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -53,6 +54,7 @@ struct smre_handle_s {
     smre_schedule schedule = SMRE_SCHED_AUTO;
     cudaGraphExec_t sweep_graph = nullptr;
     ConveyorPlan *plan = nullptr;      // null if the conveyor cannot tile this problem
+    StripPlan *strips = nullptr;       // null if the strip kernel does not take this problem
     // incomplete
     int K = 0;
     IcdLevels levels{};
@@ -135,7 +137,12 @@ extern "C" smre_status smre_create(smre_handle *out, int H, int W, int batch, co
         if (e != cudaSuccess) { smre_status s = cuda_fail(e, "allocating increment planes"); smre_destroy(h); return s; }
         smre_status s = build_sweep_graph(h);
         if (s != SMRE_OK) { smre_destroy(h); return s; }
+        // pixels outside every window of a family are never written: their increments stay 0 for the life of the handle
+        e = cudaMemset(h->q, 0, h->q_bytes);
+        if (e != cudaSuccess) { smre_status s2 = cuda_fail(e, "zeroing increment planes"); smre_destroy(h); return s2; }
         h->plan = conveyor_plan_create(H, W, batch, h->fams, h->q, h->xwork);     // may be null
+        char why[200] = "";
+        h->strips = strips_plan_create(H, W, batch, h->Wq, sides, c_table, n_sides, h->q, why, sizeof why);   // may be null
     } else {
         int K = 0;
         while ((2 << K) <= smax) ++K;
@@ -168,6 +175,7 @@ extern "C" smre_status smre_destroy(smre_handle h)
 {
     if (!h) return SMRE_OK;
     if (h->plan) conveyor_plan_destroy(h->plan);
+    if (h->strips) strips_plan_destroy(h->strips);
     if (h->sweep_graph) cudaGraphExecDestroy(h->sweep_graph);
     if (h->q) cudaFree(h->q);
     if (h->xwork) cudaFree(h->xwork);
@@ -180,8 +188,11 @@ extern "C" smre_status smre_destroy(smre_handle h)
 extern "C" smre_status smre_set_schedule(smre_handle h, smre_schedule schedule)
 {
     if (!h) return fail(SMRE_EINVAL, "handle is NULL");
-    if (schedule != SMRE_SCHED_AUTO && schedule != SMRE_SCHED_GRAPH && schedule != SMRE_SCHED_PERSISTENT)
+    if (schedule != SMRE_SCHED_AUTO && schedule != SMRE_SCHED_GRAPH && schedule != SMRE_SCHED_PERSISTENT &&
+        schedule != SMRE_SCHED_STRIPS)
         return fail(SMRE_EUNSUPPORTED, "unknown schedule %d", (int)schedule);
+    if (schedule == SMRE_SCHED_STRIPS && (h->variant != SMRE_STANDARD || !h->strips))
+        return fail(SMRE_EUNSUPPORTED, "strip schedule unavailable for this handle");
     if (schedule == SMRE_SCHED_PERSISTENT && (h->variant != SMRE_STANDARD || !h->plan))
         return fail(SMRE_EUNSUPPORTED, "persistent schedule unavailable for this handle "
                                        "(incomplete variant, or tiles do not fit on chip)");
@@ -210,6 +221,15 @@ extern "C" smre_status smre_project(smre_handle h, const float *y_dev, float *x_
         return SMRE_OK;
     }
 
+    if (h->strips && (h->schedule == SMRE_SCHED_STRIPS || h->schedule == SMRE_SCHED_AUTO)) {
+        const float *src = y_dev;
+        if (y_dev == x_out_dev) { /* in place is safe: a CTA writes rows only after their first owner has read them */ }
+        cudaError_t e = strips_run(h->strips, src, x_out_dev, n_sweeps, st, &h->last_launches);
+        if (e == cudaSuccess) { h->last_schedule = SMRE_SCHED_STRIPS; return SMRE_OK; }
+        if (h->schedule == SMRE_SCHED_STRIPS) return cuda_fail(e, "strips_run");
+        cudaGetLastError();
+        h->last_launches = 0;
+    }
     const bool persistent = h->plan && (h->schedule == SMRE_SCHED_PERSISTENT ||
                                         h->schedule == SMRE_SCHED_AUTO);
     if (persistent) {
@@ -320,6 +340,12 @@ extern "C" smre_status smre_last_launch(smre_handle h, int *schedule_used, long 
         conveyor_plan_tiles(h->plan, &ty, &tx);
         if (conveyor_plan_status(h->plan) != 0)
             return fail(SMRE_ECUDA, "conveyor scheduler: a neighbour hand-off timed out (result invalid)");
+    }
+    if (h->strips && h->last_schedule == SMRE_SCHED_STRIPS) {
+        strips_plan_shape(h->strips, &ty, &tx);
+        cudaDeviceSynchronize();
+        if (strips_plan_status(h->strips) != 0)
+            return fail(SMRE_ECUDA, "strip scheduler: a wait timed out, code 0x%x (result invalid)", strips_plan_status(h->strips));
     }
     if (tiles_y) *tiles_y = ty;
     if (tiles_x) *tiles_x = tx;

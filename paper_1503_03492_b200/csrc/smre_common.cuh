@@ -31,6 +31,15 @@ __device__ __forceinline__ float ball_scale(float n2, float c, float sqrt_c) {
 #endif
 }
 
+// The update of one pixel of a projected window (Listing 3): x' = alpha*v, q' = v - x'.
+// Written with explicit round-to-nearest operations so that no compiler contracts v - alpha*v into one fma
+// in one kernel and not in another: every scheduler and both variants round identically.
+__device__ __forceinline__ void ball_update(float v, float alpha, float &xn, float &qn)
+{
+    xn = __fmul_rn(alpha, v);
+    qn = __fsub_rn(v, xn);
+}
+
 // ---- launchers implemented in the .cu files --------------------------------------------------
 
 // smre_family.cu: one family pass over all frames (schedule SMRE_SCHED_GRAPH).  x: [B][H][W];

@@ -8,8 +8,9 @@
 // Mapping: G = next power of two >= side lanes per window, lane j owns COLUMN j of its window and
 // keeps the `side` values of that column in registers, so a warp touches 32/G neighbouring windows
 // and every row access of the warp is one contiguous segment of (32/G)*side floats (coalesced).
-// The sum of squares is a column-serial sum followed by a fixed xor-shuffle tree over the G lanes:
-// deterministic run to run.
+// The sum of squares is a column-serial sum followed by a fixed xor-shuffle tree over the G lanes,
+// neighbouring columns first: deterministic run to run, and the order the strip scheduler's sliding
+// window sums use (smre_strips.cu, window_total), so both schedulers round identically.
 #include "smre_common.cuh"
 
 namespace smre {
@@ -39,20 +40,21 @@ family_pass_kernel(float *__restrict__ x, float *__restrict__ q, int H, int W, i
     for (int r = 0; r < G; ++r) {
         v[r] = 0.0f;
         if (r < f.side && on) {
-            v[r] = x[base + (size_t)r * W] + q[qbase + (size_t)r * Wq];
+            v[r] = __fadd_rn(x[base + (size_t)r * W], q[qbase + (size_t)r * Wq]);
         }
         part = fmaf(v[r], v[r], part);
     }
 #pragma unroll
-    for (int m = G / 2; m > 0; m >>= 1) part += __shfl_xor_sync(0xffffffffu, part, m);
+    for (int m = 1; m < G; m <<= 1) part += __shfl_xor_sync(0xffffffffu, part, m);     // pairs first: (c0+c1)+(c2+c3) ...
 
     const float alpha = ball_scale(part, f.c, f.sqrt_c);
 #pragma unroll
     for (int r = 0; r < G; ++r) {
         if (r < f.side && on) {
-            const float xn = alpha * v[r];
+            float xn, qn;
+            ball_update(v[r], alpha, xn, qn);
             x[base + (size_t)r * W] = xn;
-            q[qbase + (size_t)r * Wq] = v[r] - xn;
+            q[qbase + (size_t)r * Wq] = qn;
         }
     }
 }

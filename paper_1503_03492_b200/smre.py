@@ -14,7 +14,7 @@ from . import _build
 
 SMRE_OK, SMRE_EINVAL, SMRE_EUNSUPPORTED, SMRE_ENOMEM, SMRE_ECUDA = range(5)
 SMRE_STANDARD, SMRE_INCOMPLETE = 0, 1
-SMRE_SCHED_AUTO, SMRE_SCHED_GRAPH, SMRE_SCHED_PERSISTENT = 0, 1, 2
+SMRE_SCHED_AUTO, SMRE_SCHED_GRAPH, SMRE_SCHED_PERSISTENT, SMRE_SCHED_STRIPS = 0, 1, 2, 3
 _STATUS = {0: "SMRE_OK", 1: "SMRE_EINVAL", 2: "SMRE_EUNSUPPORTED", 3: "SMRE_ENOMEM", 4: "SMRE_ECUDA"}
 
 # every symbol include/smre.h declares

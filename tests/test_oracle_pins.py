@@ -249,3 +249,32 @@ def test_transpose_equivariance_at_convergence(oracle):
     np.testing.assert_allclose(a, b, atol=1e-9)
     f = oracle.project_std(y[::-1, ::-1].copy(), sides, C(sides), 50000)[::-1, ::-1]
     np.testing.assert_allclose(a, f, atol=1e-9)
+
+
+# ---- the checker itself: t_s of every window at every shift ----------------------------
+# smre_oracle_window_sums forms the violated-window sets of the parity protocol and every feasibility pin
+# above, so it gets its own pin: an independent strided-view sum (numpy sliding_window_view, no loop of the
+# oracle retyped), the exact output shape (H-s+1, W-s+1) and the LAST row / column of windows on a ragged
+# image, whose values are chosen so that a dropped or shifted origin cannot go unnoticed.
+@pytest.mark.parametrize("H,W", [(23, 31), (8, 8), (9, 17)])
+def test_window_sums_checker_against_sliding_view(oracle, H, W):
+    from numpy.lib.stride_tricks import sliding_window_view
+    rng = np.random.default_rng(H * 100 + W)
+    x = rng.standard_normal((H, W))
+    x[-1, :] += 7.0          # the last row and column dominate every window that contains them
+    x[:, -1] -= 5.0
+    for s in range(1, min(H, W, 8) + 1):
+        got = oracle.window_sums(x, s)
+        assert got.shape == (H - s + 1, W - s + 1)
+        want = (sliding_window_view(x, (s, s)) ** 2).sum(axis=(2, 3))
+        np.testing.assert_allclose(got, want, rtol=1e-13, atol=0)
+        # origin (wy, wx) means rows wy..wy+s-1, columns wx..wx+s-1: a one-hot image has exactly s*s windows
+        # containing the pixel, at origins (r-s+1..r, c-s+1..c) clipped to the image
+        e = np.zeros((H, W))
+        r, c0 = H - 1, W - 2
+        e[r, c0] = 3.0
+        t = oracle.window_sums(e, s)
+        hit = np.argwhere(t > 0)
+        assert (t[t > 0] == 9.0).all()
+        assert hit[:, 0].min() == max(0, r - s + 1) and hit[:, 0].max() == min(r, H - s)
+        assert hit[:, 1].min() == max(0, c0 - s + 1) and hit[:, 1].max() == min(c0, W - s)
