@@ -29,6 +29,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
         if os.environ.get("SMRE_CV_TRACE_BUILD"):
             cmd.insert(1, "-DSMRE_CV_TRACE_BUILD=" + os.environ["SMRE_CV_TRACE_BUILD"])
+        if os.environ.get("SMRE_ST_KO_BUILD"):
+            cmd.insert(1, "-DSMRE_ST_KO")
         if os.environ.get("SMRE_DEBUG"):
             cmd.insert(1, "-DSMRE_DEBUG")
         else:

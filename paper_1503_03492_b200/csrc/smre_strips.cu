@@ -2,17 +2,17 @@
 // kernel runs all n_sweeps * F strictly ordered family steps (Alg. 2; order matters only for
 // overlapping sets).  Geometry: smre_strips.cuh.  Per CTA = one strip of one frame:
 //
-//   * x rows of the strip live in shared memory for the whole call (tile row = image row - j*T + 7);
+//   * the x rows of the strip live in shared memory for the whole call (tile row = image row - j*T + T/2);
 //   * compute warp k owns chunk k of every band: floor(32/s) windows, lane = image column; per family step it
 //     reads x (+ q), reduces per window (column-serial fma chain, then a fixed shuffle tree over the s lanes of
 //     the window -- the summation order of family_pass_kernel, so both schedulers agree bit for bit), scales
 //     (Eq. 14), writes x back to the tile and q to HBM; one named barrier per family step;
-//   * a loader warp streams the q rows of the strip for the coming steps from HBM into a shared-memory ring with
-//     bulk async copies (cp.async.bulk + mbarrier transaction counts), as deep as the ring allows.  The q of a
-//     pixel is always written and read by the SAME CTA (the geometry does not depend on the sweep), so there is
-//     no cross-CTA ordering of q at all; inside the CTA the loader orders a row behind its writer through
-//     `written` (release / acquire at CTA scope) and a generic->async proxy fence;
-//   * when the strip boundaries move (every macro step) the rows that change owner travel through per-CTA
+//   * two more warps stream the q rows of the coming steps from HBM into a shared-memory ring with bulk async
+//     copies (cp.async.bulk + mbarrier transaction counts), as deep as the ring allows.  The q of a pixel is always
+//     written and read by the SAME CTA (the geometry does not depend on the sweep), so there is no cross-CTA
+//     ordering of q at all; inside the CTA the copies are ordered behind the writes by the step barrier, a
+//     release / acquire pair at CTA scope and a generic->async proxy fence;
+//   * when the strip boundaries move (between macro steps) the rows that change owner travel through per-CTA
 //     mailboxes in global memory as self-validating 8-byte words {tag, value}: no fence, no flag.
 //
 // Nothing here depends on n_sweeps except the loop bound.
@@ -31,19 +31,26 @@ struct StripArgs {
     const float *y;
     float *x_out;
     float *q;                       // [F][Btot][H][Wq]
-    unsigned long long *mail_up;    // [cta][ST_RU][max_up][Wq]   written by the strip below
-    unsigned long long *mail_down;  // [cta][ST_RD][max_down][Wq] written by the strip above
+    unsigned long long *mail;       // [cta][ST_RING][tile rows][Wq] 8-byte words, written by the strips around
     unsigned *done;                 // [cta][32]: tag of the last transition this CTA has fully received
     unsigned *status;               // device word: 0 healthy, else code of the first wait that timed out
     unsigned *status_host;          // pinned host copy, written by the last CTA to finish
     unsigned *finished;             // CTAs that have finished (for status_host)
     int H, W, Wq, Btot, frame0;
-    int NS, NWC, n_sides, F, n_sweeps, NR, max_up, max_down;
+    int T, NS, NWC, n_sides, F, n_sweeps, NR, max_rows;
     int side[ST_MAX_SIDES], fam_base[ST_MAX_SIDES];
     float c[ST_MAX_SIDES], sqrt_c[ST_MAX_SIDES];
     unsigned tag_base;
     unsigned long long timeout_ns;
+#ifdef SMRE_ST_KO
+    int ko;                         // timing experiments only (wrong results): parts of the kernel switched off
+#endif
 };
+#ifdef SMRE_ST_KO
+#define ST_KO(A, bit) (((A).ko & (bit)) != 0)
+#else
+#define ST_KO(A, bit) false
+#endif
 
 // ------------------------------------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -116,7 +123,7 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 // A wait that does not come true within A.timeout_ns raises the device status word and the CTA's abort flag; from
 // then on every wait of the CTA returns at once (and other CTAs see the status word in their slow path), so a
 // protocol bug or a lost CTA ends the kernel with an error code instead of hanging the GPU.
-enum { ST_W_QFULL = 1, ST_W_QEMPTY = 2, ST_W_WRITTEN = 3, ST_W_MAIL_UP = 4, ST_W_MAIL_DOWN = 5, ST_W_DONE = 6 };
+enum { ST_W_QFULL = 1, ST_W_MAIL = 4, ST_W_DONE = 6 };
 
 struct Waiter {
     const StripArgs &A;
@@ -141,340 +148,627 @@ struct Waiter {
     }
 };
 
+// ------------------------------------------------------------------------------------------------ macro-step table
+// One entry per macro step (side index a, row offset oy) of a sweep, for THIS strip: built once at kernel start, so
+// the steady state does no geometry arithmetic (the closed forms of smre_strips.cuh need integer divisions).
+struct __align__(16) MacroEntry {
+    short s, rows, lo, nb;              // side; active rows of the strip (whole bands); first active row; bands
+    int fam0;                           // family index of (s, oy, 0)
+    float c, sqrt_c;                    // threshold of the side (Eq. 5), its square root
+    int xoff;                           // tile offset (floats) of the first active row
+    long long qoff;                     // offset (floats) of (family fam0, this frame, row lo) in the q planes
+    short hold_lo, hold_hi;             // rows the strip holds: [hold_lo, hold_hi)
+    // hand-off to the NEXT macro step (cyclic): rows [send_lo[k], send_hi[k]) go to strip j + d,
+    // d = -HOPS..-1, +1..+HOPS (k = 0..2*HOPS-1); rows [recv_lo[i], recv_hi[i]) arrive (above / below what is kept)
+    short send_lo[2 * ST_HOPS], send_hi[2 * ST_HOPS];
+    short recv_lo[2], recv_hi[2];
+    short ae_last, pad;                 // end of the last whole window of the macro step's LAST family (ox = s - 1)
+    // where each active row goes at the hand-off, 4 bits per row from `lo` on: 0 stays, 1..6 = strip j-3..j-1, j+1..j+3
+    unsigned long long sendmap;
+    long long pad2;
+};
+static_assert(sizeof(MacroEntry) == 96, "MacroEntry");
+
 // ------------------------------------------------------------------------------------------------ window sums
 // Sum over the S lanes of a window, delivered to every lane of it.  col = the lane's column sum; src = lane of the
-// window's first column.  Order: pairs, then pairs of pairs, ... = the ascending xor tree of family_pass_kernel
-// with zero padding to the next power of two, so both kernels round identically.
+// window's first column (windows start at lanes that are multiples of S).  Order: neighbouring columns first, then
+// pairs of pairs, ... = the ascending xor tree of family_pass_kernel with zero padding to the next power of two,
+// so both kernels round identically (fp addition is commutative: every lane of a power-of-two window gets the
+// same bits from the butterfly).
 template <int S>
 __device__ __forceinline__ float window_total(float col, int src)
 {
     constexpr unsigned FULL = 0xffffffffu;
     if (S == 1) return col;
+    if (S == 2 || S == 4 || S == 8) {
+        float t = col + __shfl_xor_sync(FULL, col, 1);
+        if (S >= 4) t += __shfl_xor_sync(FULL, t, 2);
+        if (S >= 8) t += __shfl_xor_sync(FULL, t, 4);
+        return t;
+    }
     const float a2 = col + __shfl_down_sync(FULL, col, 1);
-    float t = a2;
+    float t;
     if (S == 3) t = a2 + __shfl_down_sync(FULL, col, 2);
-    if (S >= 4) {
+    else {
         const float a4 = a2 + __shfl_down_sync(FULL, a2, 2);
-        t = a4;
         if (S == 5) t = a4 + __shfl_down_sync(FULL, col, 4);
-        if (S == 6) t = a4 + __shfl_down_sync(FULL, a2, 4);
-        if (S == 7) t = a4 + __shfl_down_sync(FULL, a2 + __shfl_down_sync(FULL, col, 2), 4);
-        if (S == 8) t = a4 + __shfl_down_sync(FULL, a4, 4);
+        else if (S == 6) t = a4 + __shfl_down_sync(FULL, a2, 4);
+        else t = a4 + __shfl_down_sync(FULL, a2 + __shfl_down_sync(FULL, col, 2), 4);
     }
     return __shfl_sync(FULL, t, src);
 }
 
 // ------------------------------------------------------------------------------------------------ one family step
-// xt: the lane's column in the first active tile row; qs: same place in the staged q rows (HAS_Q) ; qg: same place
-// in the family's q plane in HBM.  nb bands of S rows.  Row a2 of SURVEY.md 8(a); Eq. 14; Listing 3 PAPER.md:477-510.
-// Lanes that are not `on` (beyond the last whole window of the chunk / the image) load from a clamped, valid column
-// and take part in the shuffles, but store nothing; no active lane ever reads their values (windows are whole).
-template <int S, bool HAS_Q>
-__device__ __forceinline__ void family_step(float *xt, const float *qs, float *qg, int pitch, int Wq, int nb, bool on,
-                                            int src, float cth, float sq, int NT)
-{
-    constexpr int NBMAX = ST_MAXROWS / S;
-#pragma unroll
-    for (int b = 0; b < NBMAX; ++b) {
-        if (b < nb) {
-            float v[S];
-            float n2 = 0.0f;
-#pragma unroll
-            for (int r = 0; r < S; ++r) {
-                const int row = b * S + r;
-                const float xv = xt[row * pitch];
-                v[r] = HAS_Q ? __fadd_rn(xv, qs[row * pitch]) : xv;
-                n2 = fmaf(v[r], v[r], n2);
-            }
-            const float tot = window_total<S>(n2, src);
-            const float alpha = ball_scale(tot, cth, sq);
-            if (on) {
-#pragma unroll
-                for (int r = 0; r < S; ++r) {
-                    float xn, qn;
-                    ball_update(v[r], alpha, xn, qn);
-                    xt[(b * S + r) * pitch] = xn;
-                    __stcs(qg + (size_t)((b * S + r) * Wq), qn);
-                }
-            }
-        }
-    }
-    bar_sync(1, NT);                 // every window of the next family overlaps windows of other warps
-}
-
-// ------------------------------------------------------------------------------------------------ compute side
+// G bands of S rows starting at tile row xt / staged row qs / plane row qg (all at the lane's column).  Band 0 is
+// always there; bands >= nvalid load nothing and store nothing; lanes that are not `on` (their window is not fully
+// inside the image, or beyond the chunk) load whatever lies at their address -- always inside shared memory -- and
+// take part in the shuffles, but store nothing, and no active lane ever reads their values (windows are whole).
+// Row a2 of SURVEY.md 8(a); Eq. 14; Listing 3 PAPER.md:477-510.
+// Hand-off word {tag, value}: self-validating, so a row needs neither a fence nor a flag.
 __device__ __forceinline__ unsigned long long pack_word(unsigned tag, float v)
 {
     return ((unsigned long long)tag << 32) | (unsigned long long)__float_as_uint(v);
 }
 
+// In the LAST family of a macro step (sm != 0) the rows that change owner afterwards leave straight from the
+// registers: sm holds 4 bits per row of the group (see MacroEntry::sendmap), mb points at the lane's column of the
+// group's first row in the slot of the coming transition in MY mailbox (strip j + d: + d * dest_step).
+template <int S, int G, bool HAS_Q, int PITCH>
+__device__ __forceinline__ void band_group(float *xt, const float *qs, float *qg, int pitch_rt, int nvalid, bool on,
+                                           int src, float cth, float sq, int ko, unsigned long long sm,
+                                           unsigned long long *mb, long long dest_step, unsigned tag)
+{
+    const int pitch = PITCH ? PITCH : pitch_rt;
+    float v[G][S], n2[G], al[G];
+#pragma unroll
+    for (int i = 0; i < G; ++i) {
+        const bool pb = i == 0 || i < nvalid;
+        n2[i] = 0.0f;
+#pragma unroll
+        for (int r = 0; r < S; ++r) {
+            float xv = 0.0f, qv = 0.0f;
+            if (pb) {
+                xv = xt[(i * S + r) * pitch];
+                if (HAS_Q) qv = qs[(i * S + r) * pitch];
+            }
+            v[i][r] = HAS_Q ? __fadd_rn(xv, qv) : xv;
+            n2[i] = fmaf(v[i][r], v[i][r], n2[i]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < G; ++i) al[i] = ball_scale(window_total<S>(n2[i], src), cth, sq);
+#pragma unroll
+    for (int i = 0; i < G; ++i) {
+        if (on && (i == 0 || i < nvalid)) {
+#pragma unroll
+            for (int r = 0; r < S; ++r) {
+                float xn, qn;
+                ball_update(v[i][r], al[i], xn, qn);
+                xt[(i * S + r) * pitch] = xn;
+                if (!(ko & 4)) __stcs(qg + (i * S + r) * pitch, qn);
+                if (sm != 0) {
+                    const int code = (int)(sm >> (4 * (i * S + r))) & 15;
+                    if (code) st_relaxed_gpu64(mb + (long long)(code - 4 + (code >= 4)) * dest_step + (i * S + r) * pitch,
+                                               pack_word(tag, xn));
+                }
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ compute side
+
+// q ring: where the rows of the next staged step go.  A pure function of the sequence of row counts, so the issuer
+// and the compute warps derive the same positions independently.  A step's rows never wrap (immediate offsets).
+__device__ __forceinline__ int ring_place(int &pos, int rows, int NR)
+{
+    if (pos + rows > NR) pos = 0;
+    const int at = pos;
+    pos += rows;
+    return at;
+}
+
 struct ComputeState {
-    int g = 0;            // family steps done
-    int pos = 0;          // q ring: next free row
-    unsigned n = 0;       // staged (non-empty) steps consumed so far
-    unsigned mc = 0;      // transitions done
-    unsigned done_up, done_down;    // cached progress of the strip above / below (flow control of the mailbox rings)
+#ifdef SMRE_ST_KO
+    long long t_send = 0, t_recv = 0, t_bar = 0, t_macro = 0, t_last = 0;
+#endif
+    int pos = 0;                        // q ring: next free row
+    unsigned mc = 0;                    // transitions done
+    unsigned seen_m3, seen_m2, seen_m1, seen_p1, seen_p2, seen_p3;   // cached progress words of the strips around
+                                                                     // (flow control of their mailbox rings)
 };
 
-// Rows change owner between the families (s, oy, *) and (s2, oy2, *).  All compute threads of the CTA take part;
-// on entry every tile write of the last step is visible (step barrier), on exit the tile holds the new row set.
-// Sends come first and wait for nothing but ring space, so the hand-offs of one transition cannot form a cycle.
-__device__ __forceinline__ void transition(const StripArgs &A, float *tile, int pitch, int j, int cta, int s, int oy,
-                                           int s2, int oy2, ComputeState &cs, int tid, int NT, unsigned *written,
-                                           Waiter &w)
+// Mailbox slot of transition number mc in the mailbox of the strip of CTA `cta`, addressed by image row / column:
+// word of (row y, column c) = base[y * Wq + c]; the same slot of strip j + d lies d * st_dest_step() further on.
+__device__ __forceinline__ unsigned long long *st_mailbox(const StripArgs &A, int cta, int j, unsigned mc)
 {
-    const int NS = A.NS, H = A.H, W = A.W, Wq = A.Wq;
-    const int bt = st_boundary(j, NS, H, s, oy), bt2 = st_boundary(j, NS, H, s2, oy2);
-    const int bb = st_boundary(j + 1, NS, H, s, oy), bb2 = st_boundary(j + 1, NS, H, s2, oy2);
+    const long long slot_words = (long long)st_tile_rows(A.T) * A.Wq;
+    return A.mail + ((long long)cta * ST_RING + mc % ST_RING) * slot_words + (long long)(A.T / 2 - j * A.T) * A.Wq;
+}
+__device__ __forceinline__ long long st_dest_step(const StripArgs &A)
+{
+    return (long long)ST_RING * st_tile_rows(A.T) * A.Wq - (long long)A.T * A.Wq;
+}
+
+// Flow control of the mailbox rings: before strip j + d's slot of transition `tag` is written, that strip must have
+// read the slot's previous message (transition tag - ST_RING).  `seen` is a cached copy of its progress word,
+// refreshed at every transition without waiting, so this almost never has to wait.
+__device__ __forceinline__ void st_ring_space(const StripArgs &A, int cta, int d, unsigned tag, unsigned mc, unsigned &seen,
+                                              Waiter &w)
+{
+    if (mc <= (unsigned)ST_RING || (int)(tag - ST_RING - seen) <= 0 || ST_KO(A, 128)) return;
+    w.begin();
+    do {
+        seen = ld_relaxed_gpu32(A.done + (size_t)(cta + d) * 32);
+    } while ((int)(tag - ST_RING - seen) > 0 && !w.slow(ST_W_DONE));
+}
+
+// Rows change owner between macro step e (just finished) and the next one; e holds the plan.  All compute threads
+// of the CTA take part; on entry every tile write of the last step is visible (step barrier), on exit the tile holds
+// the new row set.  Most departing values have already left, straight from the registers of the macro step's last
+// family (band_group); here only what that family did not touch is sent: rows outside the active rows (image top /
+// bottom) and the columns outside its windows (left / right remainder).  Sends wait for nothing but ring space, so
+// the hand-offs of one transition cannot form a cycle.  A thread owns column tid (W <= compute threads).
+// A row travels to slot (receiver's tile row) of the receiver's mailbox, whoever sends it.
+__device__ __forceinline__ void transition(const StripArgs &A, float *tile, int pitch, int j, int cta,
+                                           const MacroEntry &e, ComputeState &cs, int tid, int NT, Waiter &w)
+{
+    constexpr int MAXR = 8;                                    // rows requested at once
+    static_assert(ST_HOPS == 3, "the sends below are written out for three hops");
+    const int NS = A.NS, Wq = A.Wq, T = A.T;
     const unsigned mc = ++cs.mc;
     const unsigned tag = A.tag_base + mc;
-    const int slot_base = ST_SLOT_OFF - j * ST_T;
+    if (ST_KO(A, 1)) { bar_sync(2, NT); return; }
+#ifdef SMRE_ST_KO
+    const long long c0 = clock64();
+    cs.t_macro += c0 - cs.t_last;
+#endif
+    const bool mine = tid < A.W;
+    float *tcol = tile + (T / 2 - j * T) * pitch + tid;         // tcol[y * pitch]: image row y, my column
+    unsigned long long *box = st_mailbox(A, cta, j, mc) + tid;
+    const long long dest_step = st_dest_step(A);
 
-    if (j >= 1 && bt2 > bt) {                                  // my top rows go to the strip above
-        if (mc > (unsigned)ST_RU) {
-            w.begin();
-            while ((int)(tag - ST_RU - cs.done_up) > 0) {
-                cs.done_up = ld_relaxed_gpu32(A.done + (size_t)(cta - 1) * 32);
-                if ((int)(tag - ST_RU - cs.done_up) > 0 && w.slow(ST_W_DONE)) break;
+    // progress of the strips around, for the flow control of the NEXT transition: requested now, used at the end
+    const int up1 = j >= 1, up2 = j >= 2 ? 2 : up1, up3 = j >= 3 ? 3 : up2;
+    const int dn1 = j + 1 < NS, dn2 = j + 2 < NS ? 2 : dn1, dn3 = j + 3 < NS ? 3 : dn2;
+    const unsigned s_m1 = ld_relaxed_gpu32(A.done + (size_t)(cta - up1) * 32);
+    const unsigned s_p1 = ld_relaxed_gpu32(A.done + (size_t)(cta + dn1) * 32);
+    const unsigned s_m2 = ld_relaxed_gpu32(A.done + (size_t)(cta - up2) * 32);
+    const unsigned s_p2 = ld_relaxed_gpu32(A.done + (size_t)(cta + dn2) * 32);
+    const unsigned s_m3 = ld_relaxed_gpu32(A.done + (size_t)(cta - up3) * 32);
+    const unsigned s_p3 = ld_relaxed_gpu32(A.done + (size_t)(cta + dn3) * 32);
+
+    // departures the last family did not make: whole rows outside the active rows, and my column of the active
+    // rows if it lay outside that family's windows
+    const int act_lo = e.lo, act_hi = e.lo + e.rows;
+    const bool idle_col = tid < e.s - 1 || tid >= e.ae_last;
+    auto send = [&](int d, int lo, int hi, unsigned &seen) {
+        if (lo >= hi) return;
+        st_ring_space(A, cta, d, tag, mc, seen, w);
+        if (!mine) return;
+        unsigned long long *dst = box + d * dest_step;
+        for (int y = lo; y < hi; ++y)
+            if (idle_col || y < act_lo || y >= act_hi) st_relaxed_gpu64(dst + y * Wq, pack_word(tag, tcol[y * pitch]));
+    };
+    send(-1, e.send_lo[2], e.send_hi[2], cs.seen_m1);
+    send(+1, e.send_lo[3], e.send_hi[3], cs.seen_p1);
+    send(-2, e.send_lo[1], e.send_hi[1], cs.seen_m2);
+    send(+2, e.send_lo[4], e.send_hi[4], cs.seen_p2);
+    send(-3, e.send_lo[0], e.send_hi[0], cs.seen_m3);
+    send(+3, e.send_lo[5], e.send_hi[5], cs.seen_p3);
+#ifdef SMRE_ST_KO
+    const long long c1 = clock64();
+#endif
+    // arrivals: all words of a batch are requested at once, then re-requested until their tag is right
+    const int n0 = e.recv_hi[0] - e.recv_lo[0], n1 = e.recv_hi[1] - e.recv_lo[1];
+    if (mine && n0 + n1 > 0) {
+        w.begin();
+        for (int r0 = 0; r0 < n0 + n1; r0 += MAXR) {
+            int yy[MAXR];
+            unsigned long long wd[MAXR];
+#pragma unroll
+            for (int r = 0; r < MAXR; ++r) {
+                const int i = r0 + r;
+                yy[r] = i < n0 ? e.recv_lo[0] + i : i < n0 + n1 ? e.recv_lo[1] + (i - n0) : -1;
             }
-        }
-        unsigned long long *dst = A.mail_up + ((size_t)(cta - 1) * ST_RU + mc % ST_RU) * A.max_up * Wq;
-        for (int y = bt; y < bt2; ++y)
-            for (int c = tid; c < W; c += NT)
-                st_relaxed_gpu64(dst + (size_t)(y - bt) * Wq + c, pack_word(tag, tile[(y + slot_base) * pitch + c]));
-    }
-    if (j + 1 < NS && bb2 < bb) {                              // my bottom rows go to the strip below
-        if (mc > (unsigned)ST_RD) {
-            w.begin();
-            while ((int)(tag - ST_RD - cs.done_down) > 0) {
-                cs.done_down = ld_relaxed_gpu32(A.done + (size_t)(cta + 1) * 32);
-                if ((int)(tag - ST_RD - cs.done_down) > 0 && w.slow(ST_W_DONE)) break;
-            }
-        }
-        unsigned long long *dst = A.mail_down + ((size_t)(cta + 1) * ST_RD + mc % ST_RD) * A.max_down * Wq;
-        for (int y = bb2; y < bb; ++y)
-            for (int c = tid; c < W; c += NT)
-                st_relaxed_gpu64(dst + (size_t)(y - bb2) * Wq + c, pack_word(tag, tile[(y + slot_base) * pitch + c]));
-    }
-    if (j + 1 < NS && bb2 > bb) {                              // rows arriving from below
-        const unsigned long long *src = A.mail_up + ((size_t)cta * ST_RU + mc % ST_RU) * A.max_up * Wq;
-        for (int y = bb; y < bb2; ++y)
-            for (int c = tid; c < W; c += NT) {
-                const unsigned long long *p = src + (size_t)(y - bb) * Wq + c;
-                unsigned long long wd = ld_relaxed_gpu64(p);
-                w.begin();
-                while ((unsigned)(wd >> 32) != tag) {
-                    if (w.slow(ST_W_MAIL_UP)) break;
-                    wd = ld_relaxed_gpu64(p);
+            unsigned missing;
+            int tries = 0;
+            do {
+                if (tries++ && w.slow(ST_W_MAIL)) {
+#ifdef SMRE_ST_KO
+                    if (tid < 40 || (tid & 31) == 0)
+                        printf("MAIL timeout strip %d tid %d mc %u tag %u rows [%d,%d)+[%d,%d) missing %x got tags %u %u\n", j, tid, mc, tag,
+                               e.recv_lo[0], e.recv_hi[0], e.recv_lo[1], e.recv_hi[1], missing, (unsigned)(wd[0] >> 32), (unsigned)(wd[1] >> 32));
+#endif
+                    break;
                 }
-                tile[(y + slot_base) * pitch + c] = __uint_as_float((unsigned)wd);
-            }
+#pragma unroll
+                for (int r = 0; r < MAXR; ++r)
+                    if (yy[r] >= 0) wd[r] = ld_relaxed_gpu64(box + yy[r] * Wq);
+                missing = 0;
+#pragma unroll
+                for (int r = 0; r < MAXR; ++r)
+                    if (yy[r] >= 0 && (unsigned)(wd[r] >> 32) != tag) missing |= 1u << r;
+                if (ST_KO(A, 64)) missing = 0;
+            } while (missing);
+#pragma unroll
+            for (int r = 0; r < MAXR; ++r)
+                if (yy[r] >= 0) tcol[yy[r] * pitch] = __uint_as_float((unsigned)wd[r]);
+        }
     }
-    if (j >= 1 && bt2 < bt) {                                  // rows arriving from above
-        const unsigned long long *src = A.mail_down + ((size_t)cta * ST_RD + mc % ST_RD) * A.max_down * Wq;
-        for (int y = bt2; y < bt; ++y)
-            for (int c = tid; c < W; c += NT) {
-                const unsigned long long *p = src + (size_t)(y - bt2) * Wq + c;
-                unsigned long long wd = ld_relaxed_gpu64(p);
-                w.begin();
-                while ((unsigned)(wd >> 32) != tag) {
-                    if (w.slow(ST_W_MAIL_DOWN)) break;
-                    wd = ld_relaxed_gpu64(p);
-                }
-                tile[(y + slot_base) * pitch + c] = __uint_as_float((unsigned)wd);
-            }
-    }
-    bar_sync(1, NT);
-    if (tid == 0) {
-        st_relaxed_gpu32(A.done + (size_t)cta * 32, tag);       // my mailbox slots of this transition are free again
-        st_release_cta(written, (unsigned)cs.g);                // q of every step < g is on its way to HBM (loader: acquire)
-    }
+#ifdef SMRE_ST_KO
+    const long long c2 = clock64();
+#endif
+    bar_sync(2, NT);
+    if (tid == 0) st_relaxed_gpu32(A.done + (size_t)cta * 32, tag);   // my mailbox slot of this transition is free again
+    cs.seen_m1 = s_m1; cs.seen_p1 = s_p1; cs.seen_m2 = s_m2; cs.seen_p2 = s_p2; cs.seen_m3 = s_m3; cs.seen_p3 = s_p3;
+#ifdef SMRE_ST_KO
+    const long long c3 = clock64();
+    cs.t_send += c1 - c0; cs.t_recv += c2 - c1; cs.t_bar += c3 - c2; cs.t_last = c3;
+#endif
 }
 
 // One macro step: the S families (S, oy, 0..S-1) on the strip's bands; the strip interacts with nobody meanwhile.
-template <int S>
-__device__ __forceinline__ void macro_step(const StripArgs &A, int a, int oy, bool staged, float *tile, const float *ring,
-                                           uint64_t *full, uint64_t *empty, int pitch, int Wq, int j, int frame,
-                                           ComputeState &cs, int warp, int lane, int NT, Waiter &wt)
+// One named barrier per family step (compute warps + the waiter warp): every window of the next family overlaps
+// windows of this one that other warps own.
+template <int S, int G, bool HAS_Q, int PITCH>
+__device__ __forceinline__ void macro_steps(const StripArgs &A, const MacroEntry &e, float *tile, const float *ring,
+                                            int j, int cta, ComputeState &cs, int warp, int lane, int NTL, bool handoff,
+                                            Waiter &w)
 {
     constexpr int CW = (32 / S) * S;
-    const int H = A.H, W = A.W, NS = A.NS;
+    const int pitch = PITCH ? PITCH : A.Wq;
+    const int W = A.W, NR = A.NR;
     const int src = (lane / S) * S;
-    const float cth = A.c[a], sq = A.sqrt_c[a];
-    int lo, hi;
-    st_active_rows(j, NS, H, S, oy, lo, hi);
-    const int rows = hi - lo;
-    const int nb = rows / S;
-    float *xrow = tile + (lo - j * ST_T + ST_SLOT_OFF) * pitch;
-    const float *qplane = A.q + ((size_t)(A.fam_base[a] + oy * S) * A.Btot + frame) * ((size_t)H * Wq) + (size_t)lo * Wq;
-    const size_t fam_stride = (size_t)A.Btot * H * Wq;
+    const float cth = e.c, sq = e.sqrt_c;
+    const int rows = e.rows, nb = e.nb;
+#ifdef SMRE_ST_KO
+    const int ko = A.ko;
+#else
+    constexpr int ko = 0;
+#endif
+    const int col0 = warp * CW + lane;
+    int w_end = lane < CW ? warp * CW + src + S : (1 << 28);   // end of the lane's window at ox = 0
+    float *xt = tile + e.xoff + col0;
+    float *qg = A.q + e.qoff + col0;
+    const size_t q_step = (size_t)A.Btot * A.H * pitch + 1;    // next family's plane, next column
+    const float *qcol = ring + col0;
+    const unsigned long long sendmap = (handoff && !ST_KO(A, 1)) ? e.sendmap : 0ull;
+    const unsigned tag_next = A.tag_base + cs.mc + 1;
+    const long long dest_step = st_dest_step(A);
 #pragma unroll 1
     for (int ox = 0; ox < S; ++ox) {
-        const int c = ox + warp * CW + lane;
-        const bool on = (lane < CW) && (c < ox + ((W - ox) / S) * S);
-        const int cl = c < W ? c : W - 1;                      // clamped: a valid column for the lanes that are off
-        float *qg = const_cast<float *>(qplane) + (size_t)ox * fam_stride + cl;
-        if (staged && rows > 0) {
-            if (cs.pos + rows > A.NR) cs.pos = 0;
-            const float *qs = ring + cs.pos * pitch + cl;
-            cs.pos += rows;
-            const unsigned stage = cs.n % ST_NSTG, parity = (cs.n / ST_NSTG) & 1u;
-            ++cs.n;
-            if (!mbar_try_wait(&full[stage], parity)) {
-                wt.begin();
-                while (!mbar_try_wait(&full[stage], parity))
-                    if (wt.slow(ST_W_QFULL)) break;
-            }
-            family_step<S, true>(xrow + cl, qs, qg, pitch, Wq, nb, on, src, cth, sq, NT);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[stage]);          // the staged rows have been read
-        } else {
-            family_step<S, false>(xrow + cl, nullptr, qg, pitch, Wq, nb, on, src, cth, sq, NT);
+        const bool on = w_end <= W;                            // the window lies inside the image (reading A6)
+        const float *qs = HAS_Q ? qcol + ring_place(cs.pos, rows, NR) * pitch : nullptr;
+        unsigned long long sm = 0;
+        unsigned long long *mb = nullptr;
+        if (ox == S - 1 && sendmap != 0) {                     // last family: departing rows leave from the registers
+            sm = sendmap;
+            mb = st_mailbox(A, cta, j, cs.mc + 1) + (long long)e.lo * pitch + (col0 + ox);
+            if (e.send_lo[2] < e.send_hi[2]) st_ring_space(A, cta, -1, tag_next, cs.mc + 1, cs.seen_m1, w);
+            if (e.send_lo[3] < e.send_hi[3]) st_ring_space(A, cta, +1, tag_next, cs.mc + 1, cs.seen_p1, w);
+            if (e.send_lo[1] < e.send_hi[1]) st_ring_space(A, cta, -2, tag_next, cs.mc + 1, cs.seen_m2, w);
+            if (e.send_lo[4] < e.send_hi[4]) st_ring_space(A, cta, +2, tag_next, cs.mc + 1, cs.seen_p2, w);
+            if (e.send_lo[0] < e.send_hi[0]) st_ring_space(A, cta, -3, tag_next, cs.mc + 1, cs.seen_m3, w);
+            if (e.send_lo[5] < e.send_hi[5]) st_ring_space(A, cta, +3, tag_next, cs.mc + 1, cs.seen_p3, w);
         }
-        ++cs.g;
+        if (!(ko & 8)) {
+            band_group<S, G, HAS_Q, PITCH>(xt, qs, qg, pitch, nb, on, src, cth, sq, ko, sm, mb, dest_step, tag_next);
+            for (int b0 = G; b0 < nb; b0 += G)                 // strips taller than one group
+                band_group<S, G, HAS_Q, PITCH>(xt + b0 * S * pitch, HAS_Q ? qs + b0 * S * pitch : nullptr,
+                                               qg + b0 * S * pitch, pitch, nb - b0, on, src, cth, sq, ko,
+                                               sm >> (4 * b0 * S), mb + b0 * S * pitch, dest_step, tag_next);
+        }
+        ++w_end;
+        ++xt;
+        ++qcol;
+        qg += q_step;
+        if (!(ko & 16)) bar_sync(1, NTL);
     }
 }
 
-// ------------------------------------------------------------------------------------------------ q loader warp
-template <int PITCH>
-__device__ void loader_warp(const StripArgs &A, float *ring, uint64_t *full, uint64_t *empty, unsigned *written,
-                            unsigned *abort_flag, unsigned short *qpos, unsigned short *qrows, int j, int frame, int lane)
+template <int S, int PITCH>
+__device__ __forceinline__ void macro_step(const StripArgs &A, const MacroEntry &e, bool staged, float *tile,
+                                           const float *ring, int j, int cta, ComputeState &cs, int warp, int lane,
+                                           int NTL, bool handoff, Waiter &w)
 {
-    const int pitch = PITCH ? PITCH : A.Wq;
-    const int Wq = PITCH ? PITCH : A.Wq;
-    const int H = A.H, NS = A.NS;
-    const size_t plane = (size_t)H * Wq;
-    const uint32_t row_bytes = (uint32_t)Wq * 4u;
+    constexpr int GM = S == 1 ? 4 : 2;                         // bands handled together when there are several
+    if (e.rows == 0) {                                         // nothing of this strip is inside a window row
+        for (int ox = 0; ox < S; ++ox)
+            if (!ST_KO(A, 16)) bar_sync(1, NTL);
+        return;
+    }
+    if (S == ST_MAX_SIDE || e.rows == S) {
+        if (staged) macro_steps<S, 1, true, PITCH>(A, e, tile, ring, j, cta, cs, warp, lane, NTL, handoff, w);
+        else macro_steps<S, 1, false, PITCH>(A, e, tile, ring, j, cta, cs, warp, lane, NTL, handoff, w);
+    } else {
+        if (staged) macro_steps<S, GM, true, PITCH>(A, e, tile, ring, j, cta, cs, warp, lane, NTL, handoff, w);
+        else macro_steps<S, GM, false, PITCH>(A, e, tile, ring, j, cta, cs, warp, lane, NTL, handoff, w);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ q streaming
+// Two warps besides the compute warps:
+//   * the WAITER takes part in the step barrier.  Before arriving at the barrier of step g it waits (mbarrier) until
+//     the q rows of step g + 1 have landed, so the compute warps never wait for q themselves; after the barrier it
+//     publishes progress = g + 1 with release semantics: by then every compute warp has read the staged rows of
+//     step g and issued its q stores of step g (the barrier orders both at CTA scope).
+//   * the ISSUER is decoupled: it walks the step sequence ahead of everybody and issues the bulk copies of whole
+//     batches of steps (up to 32 rows = one copy per lane), as far ahead as the ring, the stage count and the
+//     one-sweep dependency (the rows of step h were written in step h - F) allow.  It reads `progress` with acquire
+//     semantics and orders its async-proxy reads behind the generic-proxy writes with a proxy fence.
+__device__ void waiter_warp(const StripArgs &A, const MacroEntry *tab, int M, uint64_t *full, unsigned *progress,
+                            unsigned *abort_flag, int lane, int NTL)
+{
     Waiter wt(A, abort_flag);
-    int pos = 0;
-    unsigned n = 0, nt = 0;                 // issued / released stage counters
-    unsigned have = 0;                      // last value read from `written`
-    int g = A.F;
-    for (int sweep = 1; sweep < A.n_sweeps; ++sweep)
-        for (int a = 0; a < A.n_sides; ++a) {
-            const int s = A.side[a];
-            for (int oy = 0; oy < s; ++oy) {
-                int lo, hi;
-                st_active_rows(j, NS, H, s, oy, lo, hi);
-                const int rows = hi - lo;
-                for (int ox = 0; ox < s; ++ox, ++g) {
-                    if (rows == 0) continue;
-                    // (1) the rows were written one sweep ago, in step g - F: wait until the compute warps say so
-                    const unsigned need = (unsigned)(g - A.F + 1);
-                    if (have < need) {
+    const bool off = ST_KO(A, 2);
+    const int total = A.n_sweeps * A.F;
+    unsigned cn = 0;                           // staged non-empty steps consumed
+    int g = 0;
+#ifdef SMRE_ST_KO
+    long long t_wait = 0, t_bar = 0; int n_late = 0;
+#endif
+    for (int sweep = 0; sweep < A.n_sweeps; ++sweep)
+        for (int m = 0; m < M; ++m) {
+            const int crows = tab[m].rows, cs_ = tab[m].s;
+            const int nrows_macro = tab[(m + 1 == M) ? 0 : m + 1].rows;
+            const bool cur_staged = sweep > 0 && crows > 0 && !off;
+            for (int ox = 0; ox < cs_; ++ox, ++g) {
+                const bool last_ox = ox + 1 == cs_;
+                const int nrows = last_ox ? nrows_macro : crows;
+                const bool nstaged = (last_ox && m + 1 == M) ? true : sweep > 0;
+                if (!off && g + 1 < total && nstaged && nrows > 0) {
+                    const unsigned n1 = cn + (cur_staged ? 1u : 0u);
+                    const unsigned stage = n1 % ST_NSTG, parity = (n1 / ST_NSTG) & 1u;
+#ifdef SMRE_ST_KO
+                    const long long w0 = clock64();
+#endif
+                    if (!mbar_try_wait(&full[stage], parity)) {
+#ifdef SMRE_ST_KO
+                        ++n_late;
+#endif
                         wt.begin();
-                        while ((have = ld_acquire_cta(written)) < need)
-                            if (wt.slow(ST_W_WRITTEN)) break;
+                        while (!mbar_try_wait(&full[stage], parity))
+                            if (wt.slow(ST_W_QFULL)) break;
                     }
-                    // (2) ring space: positions are a function of the step sequence alone (the compute warps
-                    //     derive the same ones); wait until every older stage overlapping the new rows is released
-                    const bool wrapped = pos + rows > A.NR;
-                    const int npos = wrapped ? 0 : pos;
-                    while (nt < n) {
-                        const int fp = qpos[nt & 63u], fr = qrows[nt & 63u];
-                        const bool need_pop = (n - nt >= (unsigned)ST_NSTG) || (fp < npos + rows && npos < fp + fr) ||
-                                              (wrapped && fp >= pos);
-                        if (!need_pop) break;
-                        const unsigned stage = nt % ST_NSTG, parity = (nt / ST_NSTG) & 1u;
-                        if (!mbar_try_wait(&empty[stage], parity)) {
-                            wt.begin();
-                            while (!mbar_try_wait(&empty[stage], parity))
-                                if (wt.slow(ST_W_QEMPTY)) break;
-                        }
-                        ++nt;
-                    }
-                    __syncwarp();
-                    if (lane == 0) { qpos[n & 63u] = (unsigned short)npos; qrows[n & 63u] = (unsigned short)rows; }
-                    // (3) order the async-proxy reads behind the generic-proxy writes acquired in (1), then issue
-                    fence_proxy_async();
-                    uint64_t *bar = &full[n % ST_NSTG];
-                    if (lane == 0) mbar_arrive_expect_tx(bar, (uint32_t)rows * row_bytes);
-                    __syncwarp();
-                    const float *srcp = A.q + ((size_t)(A.fam_base[a] + oy * s + ox) * A.Btot + frame) * plane +
-                                        (size_t)lo * Wq;
-                    for (int r = lane; r < rows; r += 32)
-                        bulk_load_row(ring + (size_t)(npos + r) * pitch, srcp + (size_t)r * Wq, row_bytes, bar);
-                    pos = npos + rows;
-                    ++n;
+#ifdef SMRE_ST_KO
+                    t_wait += clock64() - w0;
+#endif
                 }
+#ifdef SMRE_ST_KO
+                const long long b0 = clock64();
+#endif
+                if (!ST_KO(A, 16)) bar_sync(1, NTL);
+                if (cur_staged) ++cn;
+                if (lane == 0) st_release_cta(progress, (unsigned)(g + 1));
+#ifdef SMRE_ST_KO
+                t_bar += clock64() - b0;
+#endif
             }
         }
+#ifdef SMRE_ST_KO
+    if ((A.ko & 256) && lane == 0 && (blockIdx.x % 40) == 3)
+        printf("waiter cta %d: steps %d  q-wait %lld cycles/step  late %d  barrier+release %lld cycles/step\n", blockIdx.x, g,
+               t_wait / max(g, 1), n_late, t_bar / max(g, 1));
+#endif
+}
+
+// Position in the sequence of STAGED (sweep >= 1), NON-EMPTY steps, with the ring_place state before the step.
+struct StagedCursor {
+    int m = 0, ox = 0;          // macro step, family inside it
+    int g;                      // global step index
+    int pos = 0;                // ring_place state before this step
+    unsigned n = 0;             // staged non-empty steps before this one
+};
+// skip macro steps in which the strip has no rows (they are not staged)
+__device__ __forceinline__ void staged_skip_empty(StagedCursor &k, const MacroEntry *tab, int M, int total)
+{
+    while (k.g < total && tab[k.m].rows == 0) {
+        k.g += tab[k.m].s - k.ox;
+        k.ox = 0;
+        if (++k.m == M) k.m = 0;
+    }
+}
+
+template <int PITCH>
+__device__ void issuer_warp(const StripArgs &A, const MacroEntry *tab, int M, float *ring, uint64_t *full,
+                            unsigned *progress, unsigned *abort_flag, int frame, int lane)
+{
+    constexpr int KMAX = 4;                                     // steps per batch (bookkeeping stays in registers)
+    const int pitch = PITCH ? PITCH : A.Wq;
+    const size_t plane = (size_t)A.H * pitch;
+    const size_t fam_stride = (size_t)A.Btot * plane;
+    const uint32_t row_bytes = (uint32_t)pitch * 4u;
+    const int NR = A.NR, F = A.F;
+    const int total = A.n_sweeps * F;
+    if (ST_KO(A, 2) || A.n_sweeps < 2) return;
+    Waiter wt(A, abort_flag);
+    StagedCursor head, tail;                   // head: next step to load; tail: oldest step not yet known to be consumed
+    head.g = tail.g = F;                       // the first staged step is step F = sweep 1, first family
+    staged_skip_empty(head, tab, M, total);
+    tail = head;
+    unsigned have = 0;                         // last value read from `progress` (= family steps completed)
+    while (head.g < total) {
+        const MacroEntry he = tab[head.m];
+        const int rows = he.rows;
+        // batch: up to 32 rows (one bulk copy per lane), inside this macro step; at most F - 1 steps, because the
+        // waiter may need the first step of the batch while only the steps before it are complete; small enough to
+        // fit the ring next to the step being consumed
+        int k = min(min(32 / rows, KMAX), he.s - head.ox);
+        k = min(k, max(1, F - 1));
+        k = min(k, total - head.g);
+        k = min(k, max(1, (NR - 2 * A.max_rows) / rows));
+        // ring rows of the batch; `gap` = rows at the end of the ring skipped by a wrap inside the batch
+        int at[KMAX];
+        int p = head.pos, gap_lo = NR;
+#pragma unroll
+        for (int i = 0; i < KMAX; ++i)
+            if (i < k) {
+                if (p + rows > NR) gap_lo = p;
+                at[i] = ring_place(p, rows, NR);
+            }
+        // what must have happened before the copies may be issued, as a count of completed family steps:
+        // (a) the batch's rows were written one sweep earlier;
+        unsigned need = (unsigned)(head.g + k - F);
+        // (b) every older step whose ring rows (or mbarrier stage) the batch takes over has been consumed
+        while (tail.g < head.g) {
+            const int trows = tab[tail.m].rows;
+            int tp = tail.pos;
+            const int tat = ring_place(tp, trows, NR);
+            bool pop = head.n + (unsigned)k - tail.n > (unsigned)ST_NSTG || tat + trows > gap_lo;
+#pragma unroll
+            for (int i = 0; i < KMAX; ++i)
+                if (i < k && tat < at[i] + rows && at[i] < tat + trows) pop = true;
+            if (!pop) break;
+            need = max(need, (unsigned)(tail.g + 1));
+            tail.pos = tp;
+            ++tail.n;
+            ++tail.g;
+            if (++tail.ox == tab[tail.m].s) { tail.ox = 0; if (++tail.m == M) tail.m = 0; }
+            staged_skip_empty(tail, tab, M, total);
+        }
+        if (have < need) {
+            wt.begin();
+            while ((have = ld_acquire_cta(progress)) < need)
+                if (wt.slow(ST_W_QFULL)) break;
+        }
+        fence_proxy_async();                                    // generic-proxy q stores -> async-proxy reads
+        if (lane < k) mbar_arrive_expect_tx(&full[(head.n + lane) % ST_NSTG], (uint32_t)rows * row_bytes);
+        __syncwarp();
+        {
+            const int i = lane / rows, r = lane - i * rows;     // lane -> (step of the batch, row of the step)
+            int my_at = at[0];
+#pragma unroll
+            for (int t = 1; t < KMAX; ++t)
+                if (t == i) my_at = at[t];
+            if (i < k) {
+                const float *src = A.q + ((size_t)(he.fam0 + head.ox + i) * A.Btot + frame) * plane +
+                                   (size_t)(he.lo + r) * pitch;
+                bulk_load_row(ring + (size_t)(my_at + r) * pitch, src, row_bytes, &full[(head.n + i) % ST_NSTG]);
+            }
+        }
+        (void)fam_stride;
+        head.pos = p;
+        head.n += (unsigned)k;
+        head.g += k;
+        head.ox += k;
+        if (head.ox == he.s) { head.ox = 0; if (++head.m == M) head.m = 0; }
+        staged_skip_empty(head, tab, M, total);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ kernel
+// MAXT = 672: 21 warps x 88 registers (96 do not fit); MAXT = 1024: 64 registers
 template <int PITCH, int MAXT>
-__global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__ StripArgs A)
+__global__ void __maxnreg__(MAXT <= 672 ? 88 : 64) strips_kernel(const __grid_constant__ StripArgs A)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int pitch = PITCH ? PITCH : A.Wq;
+    const int T = A.T, TR = st_tile_rows(T);
     float *tile = reinterpret_cast<float *>(smem_raw);
-    float *ring = tile + ST_TR * pitch;
+    float *ring = tile + TR * pitch;
     uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)A.NR * pitch);
-    uint64_t *empty = full + ST_NSTG;
-    unsigned *written = reinterpret_cast<unsigned *>(empty + ST_NSTG);
-    unsigned *abort_flag = written + 1;
-    unsigned short *qpos = reinterpret_cast<unsigned short *>(written + 2);
-    unsigned short *qrows = qpos + 64;
+    MacroEntry *tab = reinterpret_cast<MacroEntry *>(full + ST_NSTG);
+    unsigned *abort_flag = reinterpret_cast<unsigned *>(tab + ST_MAX_SIDES * ST_MAX_SIDE);
+    unsigned *progress = abort_flag + 1;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int NWC = A.NWC, NT = NWC * 32;
+    const int NWC = A.NWC, NT = NWC * 32, NTL = NT + (ST_KO(A, 32) ? 0 : 32);
     const int cta = blockIdx.x, fl = cta / A.NS, j = cta - fl * A.NS, frame = A.frame0 + fl;
     const int H = A.H, W = A.W, NS = A.NS;
 
+    // macro-step table of this strip
+    int M = 0;
+    for (int a = 0; a < A.n_sides; ++a) M += A.side[a];
+    if ((int)threadIdx.x < M) {
+        int a = 0, m0 = 0;
+        while ((int)threadIdx.x >= m0 + A.side[a]) { m0 += A.side[a]; ++a; }
+        const int s = A.side[a], oy = (int)threadIdx.x - m0;
+        int s2 = s, oy2 = oy + 1;                                // the next macro step (cyclic)
+        if (oy2 == s) { oy2 = 0; s2 = A.side[a + 1 == A.n_sides ? 0 : a + 1]; }
+        int lo, hi;
+        st_active_rows(j, NS, H, T, s, oy, lo, hi);
+        MacroEntry e;
+        e.s = (short)s; e.rows = (short)(hi - lo); e.lo = (short)lo; e.nb = (short)((hi - lo) / s);
+        e.fam0 = A.fam_base[a] + oy * s; e.c = A.c[a]; e.sqrt_c = A.sqrt_c[a];
+        e.xoff = (lo - j * T + T / 2) * pitch;
+        e.qoff = ((long long)e.fam0 * A.Btot + frame) * ((long long)H * pitch) + (long long)lo * pitch;
+        const int olo = st_boundary(j, NS, H, T, s, oy), ohi = st_boundary(j + 1, NS, H, T, s, oy);
+        const int nlo = st_boundary(j, NS, H, T, s2, oy2), nhi = st_boundary(j + 1, NS, H, T, s2, oy2);
+        e.hold_lo = (short)olo; e.hold_hi = (short)ohi;
+        for (int k = 0; k < 2 * ST_HOPS; ++k) {
+            const int d = k < ST_HOPS ? k - ST_HOPS : k - ST_HOPS + 1, jd = j + d;
+            int slo = 0, shi = 0;
+            if (jd >= 0 && jd < NS) {                            // what I hold now and strip j + d holds next
+                slo = max(olo, st_boundary(jd, NS, H, T, s2, oy2));
+                shi = min(ohi, st_boundary(jd + 1, NS, H, T, s2, oy2));
+                if (shi < slo) shi = slo;
+            }
+            e.send_lo[k] = (short)slo; e.send_hi[k] = (short)shi;
+        }
+        // what I hold next and do not hold now: above / below what I keep
+        e.recv_lo[0] = (short)nlo; e.recv_hi[0] = (short)max(nlo, min(nhi, olo));
+        e.recv_lo[1] = (short)min(nhi, max(nlo, ohi)); e.recv_hi[1] = (short)nhi;
+        e.ae_last = (short)((s - 1) + ((W - (s - 1)) / s) * s);
+        e.pad = 0; e.pad2 = 0;
+        e.sendmap = 0;
+        for (int i = 0; i < hi - lo && i < 16; ++i) {            // where the active row lo + i goes
+            const int y = lo + i;
+            for (int k = 0; k < 2 * ST_HOPS; ++k)
+                if (y >= e.send_lo[k] && y < e.send_hi[k]) e.sendmap |= (unsigned long long)(k + 1) << (4 * i);
+        }
+        tab[threadIdx.x] = e;
+    }
     if (threadIdx.x == 0) {
-        for (int i = 0; i < ST_NSTG; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], NWC); }
-        *written = 0u;
+        for (int i = 0; i < ST_NSTG; ++i) mbar_init(&full[i], 1);
         *abort_flag = 0u;
+        *progress = 0u;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
     if (warp == NWC) {
-        loader_warp<PITCH>(A, ring, full, empty, written, abort_flag, qpos, qrows, j, frame, lane);
+        if (!ST_KO(A, 32)) waiter_warp(A, tab, M, full, progress, abort_flag, lane, NTL);
+    } else if (warp == NWC + 1) {
+        issuer_warp<PITCH>(A, tab, M, ring, full, progress, abort_flag, frame, lane);
     } else {
         const int tid = threadIdx.x;
-        // row a1: x <- y for the rows of the first family's geometry (q needs no zeroing: the first sweep reads none)
+        const int slot_base = T / 2 - j * T;
+        // row a1: x <- y for the rows the strip holds under the first family's geometry (q needs no zeroing: the
+        // first sweep reads none)
         const float *yim = A.y + (size_t)frame * H * W;
-        {
-            const int lo = st_boundary(j, NS, H, A.side[0], 0), hi = st_boundary(j + 1, NS, H, A.side[0], 0);
-            for (int y = lo; y < hi; ++y)
-                for (int c = tid; c < W; c += NT) tile[(y - j * ST_T + ST_SLOT_OFF) * pitch + c] = yim[(size_t)y * W + c];
-        }
-        bar_sync(1, NT);
+        for (int y = tab[0].hold_lo; y < tab[0].hold_hi; ++y)
+            for (int c = tid; c < W; c += NT) tile[(y + slot_base) * pitch + c] = yim[(size_t)y * W + c];
+        bar_sync(2, NT);
         ComputeState cs;
-        cs.done_up = cs.done_down = A.tag_base;
+#ifdef SMRE_ST_KO
+        cs.t_last = clock64();
+#endif
+        cs.seen_m3 = cs.seen_m2 = cs.seen_m1 = cs.seen_p1 = cs.seen_p2 = cs.seen_p3 = A.tag_base;
         Waiter wt(A, abort_flag);
-        const int Wq = PITCH ? PITCH : A.Wq;
         for (int sweep = 0; sweep < A.n_sweeps; ++sweep)
-            for (int a = 0; a < A.n_sides; ++a) {
-                const int s = A.side[a];
-                for (int oy = 0; oy < s; ++oy) {
+            for (int m = 0; m < M; ++m) {
+                const MacroEntry e = tab[m];
+                const bool staged = sweep > 0 && !ST_KO(A, 2);
+                const bool handoff = !(m + 1 == M && sweep + 1 == A.n_sweeps);   // none after the very last one
 #define SMRE_RUN(S_)                                                                                                   \
-    case S_:                                                                                                           \
-        macro_step<S_>(A, a, oy, sweep > 0, tile, ring, full, empty, pitch, Wq, j, frame, cs, warp, lane, NT, wt);     \
-        break;
-                    switch (s) {
-                        SMRE_RUN(1) SMRE_RUN(2) SMRE_RUN(3) SMRE_RUN(4) SMRE_RUN(5) SMRE_RUN(6) SMRE_RUN(7) SMRE_RUN(8)
-                    }
-#undef SMRE_RUN
-                    // next macro step: (s, oy + 1), or the first one of the next side; none after the very last one
-                    int s2 = s, oy2 = oy + 1;
-                    if (oy2 == s) {
-                        if (a + 1 == A.n_sides && sweep + 1 == A.n_sweeps) break;
-                        oy2 = 0;
-                        s2 = A.side[(a + 1 == A.n_sides) ? 0 : a + 1];
-                    }
-                    transition(A, tile, pitch, j, cta, s, oy, s2, oy2, cs, tid, NT, written, wt);
+    case S_: macro_step<S_, PITCH>(A, e, staged, tile, ring, j, cta, cs, warp, lane, NTL, handoff, wt); break;
+                switch (e.s) {
+                    SMRE_RUN(1) SMRE_RUN(2) SMRE_RUN(3) SMRE_RUN(4) SMRE_RUN(5) SMRE_RUN(6) SMRE_RUN(7) SMRE_RUN(8)
                 }
+#undef SMRE_RUN
+                if (!handoff) break;
+                transition(A, tile, pitch, j, cta, e, cs, tid, NT, wt);
             }
-        // row a9: the strip's rows under the last family's geometry
-        {
-            const int s = A.side[A.n_sides - 1];
-            const int lo = st_boundary(j, NS, H, s, s - 1), hi = st_boundary(j + 1, NS, H, s, s - 1);
-            float *xo = A.x_out + (size_t)frame * H * W;
-            for (int y = lo; y < hi; ++y)
-                for (int c = tid; c < W; c += NT) xo[(size_t)y * W + c] = tile[(y - j * ST_T + ST_SLOT_OFF) * pitch + c];
-        }
+#ifdef SMRE_ST_KO
+        if ((A.ko & 256) && (tid == 0 || tid == 200) && (j == NS / 2 || j == NS / 2 + 1 || j == 3))
+            printf("strip %d tid %d: transitions %u  send %lld  recv %lld  bar %lld  macro %lld cycles (avg per transition)\n", j, tid,
+                   cs.mc, cs.t_send / max(cs.mc, 1u), cs.t_recv / max(cs.mc, 1u), cs.t_bar / max(cs.mc, 1u), cs.t_macro / max(cs.mc, 1u));
+#endif
+        // row a9: the rows the strip holds under the last family's geometry
+        float *xo = A.x_out + (size_t)frame * H * W;
+        for (int y = tab[M - 1].hold_lo; y < tab[M - 1].hold_hi; ++y)
+            for (int c = tid; c < W; c += NT) xo[(size_t)y * W + c] = tile[(y + slot_base) * pitch + c];
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -490,15 +784,15 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
 
 // ------------------------------------------------------------------------------------------------ host side
 struct StripPlan {
-    int H = 0, W = 0, B = 0, Wq = 0, NS = 0, NWC = 0, F = 0, NR = 0, max_up = 1, max_down = 1, frames_per_launch = 1;
+    int H = 0, W = 0, B = 0, Wq = 0, T = 0, NS = 0, NWC = 0, F = 0, NR = 0, max_rows = 0, frames_per_launch = 1;
     int n_sides = 0, side[ST_MAX_SIDES] = {}, fam_base[ST_MAX_SIDES] = {};
     float c[ST_MAX_SIDES] = {}, sqrt_c[ST_MAX_SIDES] = {};
     float *q = nullptr;
-    unsigned long long *mail_up = nullptr, *mail_down = nullptr;
+    unsigned long long *mail = nullptr;
     unsigned *done = nullptr, *status = nullptr, *finished = nullptr;
     unsigned *status_host = nullptr;                             // pinned, mapped
     unsigned *status_host_dev = nullptr;
-    size_t mail_up_bytes = 0, mail_down_bytes = 0, smem_bytes = 0;
+    size_t mail_bytes = 0, smem_bytes = 0;
     unsigned tag_base = 1;
     unsigned long long timeout_ns = 2000000000ull;
     int device = 0;
@@ -515,6 +809,40 @@ static void set_why(char *why, size_t n, const char *fmt, ...)
     va_end(ap);
 }
 
+static size_t strips_fixed_smem() { return ST_NSTG * 8 + ST_MAX_SIDES * ST_MAX_SIDE * sizeof(MacroEntry) + 16; }
+
+// Brute-force check of one strip height against every geometry of a sweep (host only, closed forms).
+static bool strips_check_T(int H, int NS, int T, const int *sides, int n_sides, int *max_rows, int *max_hop,
+                           char *why, size_t why_len)
+{
+    const int TR = st_tile_rows(T);
+    *max_rows = 0;
+    *max_hop = 0;
+    for (int a = 0; a < n_sides; ++a)
+        for (int oy = 0; oy < sides[a]; ++oy) {
+            int s2 = sides[a], oy2 = oy + 1;
+            if (oy2 == s2) { oy2 = 0; s2 = sides[(a + 1) % n_sides]; }
+            for (int j = 0; j < NS; ++j) {
+                int lo, hi;
+                st_active_rows(j, NS, H, T, sides[a], oy, lo, hi);
+                *max_rows = std::max(*max_rows, hi - lo);
+                const int bt = st_boundary(j, NS, H, T, sides[a], oy), bb = st_boundary(j + 1, NS, H, T, sides[a], oy);
+                if (bb > bt && (bt - j * T + T / 2 < 0 || bb - j * T + T / 2 > TR)) {
+                    set_why(why, why_len, "strip %d does not fit its tile", j);
+                    return false;
+                }
+                for (int y = bt; y < bb; ++y) {                 // who holds row y next?
+                    int j2 = j;
+                    while (j2 > 0 && y < st_boundary(j2, NS, H, T, s2, oy2)) --j2;
+                    while (j2 + 1 < NS && y >= st_boundary(j2 + 1, NS, H, T, s2, oy2)) ++j2;
+                    *max_hop = std::max(*max_hop, std::abs(j2 - j));
+                }
+            }
+        }
+    if (*max_hop > ST_HOPS) { set_why(why, why_len, "rows move %d strips at once (limit %d)", *max_hop, ST_HOPS); return false; }
+    return true;
+}
+
 bool strips_summary(int H, int W, int B, const int *sides, int n_sides, int sm_count, int smem_optin,
                     StripSummary *out, char *why, size_t why_len)
 {
@@ -524,11 +852,8 @@ bool strips_summary(int H, int W, int B, const int *sides, int n_sides, int sm_c
         if (sides[a] > ST_MAX_SIDE) { set_why(why, why_len, "side %d > %d", sides[a], ST_MAX_SIDE); return false; }
         F += sides[a] * sides[a];
     }
-    const int NS = (H + ST_T - 1) / ST_T;
-    if (NS > sm_count) {
-        set_why(why, why_len, "%d strips of %d rows need more than the %d co-resident CTAs", NS, ST_T, sm_count);
-        return false;
-    }
+    if (F < 2) { set_why(why, why_len, "a single family per sweep leaves nothing to prefetch"); return false; }
+    if (H > 32000 || W > 32000) { set_why(why, why_len, "image too large"); return false; }
     int NWC = 1;
     for (int a = 0; a < n_sides; ++a) {
         const int cw = st_chunk_width(sides[a]);
@@ -539,54 +864,39 @@ bool strips_summary(int H, int W, int B, const int *sides, int n_sides, int sm_c
         return false;
     }
     const int Wq = (W + 3) & ~3;
-    // rows per step, rows moving per transition: brute force over one sweep (closed-form geometry, host only)
-    int max_rows = 0, max_up = 1, max_down = 1;
-    for (int a = 0; a < n_sides; ++a)
-        for (int oy = 0; oy < sides[a]; ++oy) {
-            int s2 = sides[a], oy2 = oy + 1;
-            if (oy2 == s2) { oy2 = 0; s2 = sides[(a + 1) % n_sides]; }
-            for (int j = 0; j < NS; ++j) {
-                int lo, hi;
-                st_active_rows(j, NS, H, sides[a], oy, lo, hi);
-                max_rows = std::max(max_rows, hi - lo);
-                const int hold = st_boundary(j + 1, NS, H, sides[a], oy) - st_boundary(j, NS, H, sides[a], oy);
-                if (hold > ST_TR || st_boundary(j, NS, H, sides[a], oy) - j * ST_T + ST_SLOT_OFF < 0 ||
-                    st_boundary(j + 1, NS, H, sides[a], oy) - j * ST_T + ST_SLOT_OFF > ST_TR) {
-                    set_why(why, why_len, "strip %d does not fit its tile", j);
-                    return false;
-                }
-                const int b_old = st_boundary(j, NS, H, sides[a], oy), b_new = st_boundary(j, NS, H, s2, oy2);
-                const int d = b_new - b_old;
-                if (d > 0) max_up = std::max(max_up, d);
-                if (d < 0) max_down = std::max(max_down, -d);
-                // a row that changes owner goes to a neighbouring strip (single hop)
-                if ((d < 0 && b_new < st_boundary(j - 1, NS, H, sides[a], oy)) ||
-                    (d > 0 && b_new > st_boundary(j + 1, NS, H, sides[a], oy))) {
-                    set_why(why, why_len, "boundary %d moves past a whole strip", j);
-                    return false;
-                }
-            }
-        }
-    if (max_rows > ST_MAXROWS) { set_why(why, why_len, "a strip has %d active rows (limit %d)", max_rows, ST_MAXROWS); return false; }
-    const long long tile_bytes = (long long)ST_TR * Wq * 4;
-    const long long fixed = ST_NSTG * 16 + 8 + 256 + 128;
-    const long long ring_rows = (smem_optin - tile_bytes - fixed) / ((long long)Wq * 4);
-    if (ring_rows < 3 * ST_MAXROWS) {
+    // strip height: the smallest one whose strips are all co-resident (one CTA per SM): more, thinner strips mean
+    // fewer rows per CTA and step -- a strip never holds more than one band of a side >= T
+    int T = 0, NS = 0, max_rows = 0, max_hop = 0;
+    const int forced = getenv("SMRE_STRIP_T") ? atoi(getenv("SMRE_STRIP_T")) : 0;
+    for (int t : {4, 8}) {
+        if (forced && t != forced) continue;
+        const int ns = (H + t - 1) / t;
+        if (ns > sm_count) continue;
+        if (!strips_check_T(H, ns, t, sides, n_sides, &max_rows, &max_hop, why, why_len)) continue;
+        T = t; NS = ns;
+        break;
+    }
+    if (!T) {
+        if (why && !why[0]) set_why(why, why_len, "%d rows need more strips than the %d co-resident CTAs", H, sm_count);
+        return false;
+    }
+    const long long tile_bytes = (long long)st_tile_rows(T) * Wq * 4;
+    const long long ring_rows = (smem_optin - tile_bytes - (long long)strips_fixed_smem() - 128) / ((long long)Wq * 4);
+    if (ring_rows < 3 * max_rows + 8) {
         set_why(why, why_len, "shared memory holds only %lld q rows of width %d", ring_rows, W);
         return false;
     }
     if (out) {
+        out->T = T;
         out->strips = NS;
         out->warps = NWC;
         out->max_rows = max_rows;
-        out->max_up = max_up;
-        out->max_down = max_down;
-        out->ring_rows = (int)std::min<long long>(ring_rows, 60000);
+        out->max_hop = max_hop;
+        out->ring_rows = (int)std::min<long long>(ring_rows, 30000);
         out->frames_per_launch = std::max(1, std::min(B, sm_count / NS));
         const long long ctas = (long long)out->frames_per_launch * NS;
-        out->workspace_bytes = ctas * ((long long)ST_RU * max_up + (long long)ST_RD * max_down) * Wq * 8 + ctas * 128;
+        out->workspace_bytes = ctas * ST_RING * st_tile_rows(T) * Wq * 8 + ctas * 128;
     }
-    (void)F;
     return true;
 }
 
@@ -603,13 +913,14 @@ StripPlan *strips_plan_create(int H, int W, int B, int Wq, const int *sides, con
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
     if (!coop) { set_why(why, why_len, "device has no cooperative launch"); return nullptr; }
     StripSummary sm;
+    if (why && why_len) why[0] = 0;
     if (!strips_summary(H, W, B, sides, n_sides, sms, smem, &sm, why, why_len)) return nullptr;
 
     StripPlan *p = new StripPlan;
     p->device = dev;
     p->H = H; p->W = W; p->B = B; p->Wq = Wq; p->q = q;
-    p->NS = sm.strips; p->NWC = sm.warps; p->NR = sm.ring_rows;
-    p->max_up = sm.max_up; p->max_down = sm.max_down; p->frames_per_launch = sm.frames_per_launch;
+    p->T = sm.T; p->NS = sm.strips; p->NWC = sm.warps; p->NR = sm.ring_rows; p->max_rows = sm.max_rows;
+    p->frames_per_launch = sm.frames_per_launch;
     p->n_sides = n_sides;
     int F = 0;
     for (int a = 0; a < n_sides; ++a) {
@@ -617,27 +928,24 @@ StripPlan *strips_plan_create(int H, int W, int B, int Wq, const int *sides, con
         F += sides[a] * sides[a];
     }
     p->F = F;
-    p->threads = (p->NWC + 1) * 32;
+    p->threads = (p->NWC + 2) * 32;                               // compute warps + waiter + issuer
     const bool big = p->threads > 672;
     if (Wq == 512) p->kernel = big ? kernel_ptr<512, 1024>() : kernel_ptr<512, 672>();
     else p->kernel = big ? kernel_ptr<0, 1024>() : kernel_ptr<0, 672>();
-    p->smem_bytes = (size_t)ST_TR * Wq * 4 + (size_t)p->NR * Wq * 4 + ST_NSTG * 16 + 8 + 256;
+    p->smem_bytes = (size_t)st_tile_rows(p->T) * Wq * 4 + (size_t)p->NR * Wq * 4 + strips_fixed_smem();
     if (const char *e = getenv("SMRE_TIMEOUT_MS")) {
         const long long ms = atoll(e);
         if (ms > 0) p->timeout_ns = (unsigned long long)ms * 1000000ull;
     }
     const size_t ctas = (size_t)p->frames_per_launch * p->NS;
-    p->mail_up_bytes = ctas * ST_RU * p->max_up * Wq * 8;
-    p->mail_down_bytes = ctas * ST_RD * p->max_down * Wq * 8;
+    p->mail_bytes = ctas * ST_RING * st_tile_rows(p->T) * Wq * 8;
     cudaError_t e = cudaFuncSetAttribute(p->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&p->mail_up, p->mail_up_bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&p->mail_down, p->mail_down_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&p->mail, p->mail_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&p->done, ctas * 128);
     if (e == cudaSuccess) e = cudaMalloc(&p->status, 256);
     if (e == cudaSuccess) e = cudaHostAlloc(&p->status_host, 64, cudaHostAllocMapped);
     if (e == cudaSuccess) e = cudaHostGetDevicePointer(&p->status_host_dev, p->status_host, 0);
-    if (e == cudaSuccess) e = cudaMemset(p->mail_up, 0, p->mail_up_bytes);
-    if (e == cudaSuccess) e = cudaMemset(p->mail_down, 0, p->mail_down_bytes);
+    if (e == cudaSuccess) e = cudaMemset(p->mail, 0, p->mail_bytes);
     if (e == cudaSuccess) e = cudaMemset(p->done, 0, ctas * 128);
     if (e == cudaSuccess) e = cudaMemset(p->status, 0, 256);
     int nb = 0;
@@ -657,8 +965,7 @@ StripPlan *strips_plan_create(int H, int W, int B, int Wq, const int *sides, con
 void strips_plan_destroy(StripPlan *p)
 {
     if (!p) return;
-    if (p->mail_up) cudaFree(p->mail_up);
-    if (p->mail_down) cudaFree(p->mail_down);
+    if (p->mail) cudaFree(p->mail);
     if (p->done) cudaFree(p->done);
     if (p->status) cudaFree(p->status);
     if (p->status_host) cudaFreeHost(p->status_host);
@@ -678,30 +985,32 @@ cudaError_t strips_run(StripPlan *p, const float *y, float *x_out, int n_sweeps,
     int M = 0;
     for (int a = 0; a < p->n_sides; ++a) M += p->side[a];
     const unsigned long long total = (unsigned long long)n_sweeps * M + 2;
-    if (total >= 0x40000000ull) return cudaErrorNotSupported;
+    if (total >= 0x40000000ull || (unsigned long long)n_sweeps * p->F >= 0x7fffffffull) return cudaErrorNotSupported;
     cudaError_t e = cudaMemsetAsync(p->status, 0, 256, st);
     if (e != cudaSuccess) return e;
     for (int f0 = 0; f0 < p->B; f0 += p->frames_per_launch) {
         const int nf = std::min(p->frames_per_launch, p->B - f0);
         if (p->tag_base + total < p->tag_base || p->tag_base + total > 0xfffffff0u) {     // 32-bit tags used up: start over
-            e = cudaMemsetAsync(p->mail_up, 0, p->mail_up_bytes, st);
-            if (e == cudaSuccess) e = cudaMemsetAsync(p->mail_down, 0, p->mail_down_bytes, st);
+            e = cudaMemsetAsync(p->mail, 0, p->mail_bytes, st);
             if (e == cudaSuccess) e = cudaMemsetAsync(p->done, 0, (size_t)p->frames_per_launch * p->NS * 128, st);
             if (e != cudaSuccess) return e;
             p->tag_base = 1;
         }
         StripArgs A{};
         A.y = y; A.x_out = x_out; A.q = p->q;
-        A.mail_up = p->mail_up; A.mail_down = p->mail_down; A.done = p->done;
+        A.mail = p->mail; A.done = p->done;
         A.status = p->status; A.status_host = p->status_host_dev; A.finished = p->finished;
         A.H = p->H; A.W = p->W; A.Wq = p->Wq; A.Btot = p->B; A.frame0 = f0;
-        A.NS = p->NS; A.NWC = p->NWC; A.n_sides = p->n_sides; A.F = p->F; A.n_sweeps = n_sweeps; A.NR = p->NR;
-        A.max_up = p->max_up; A.max_down = p->max_down;
+        A.T = p->T; A.NS = p->NS; A.NWC = p->NWC; A.n_sides = p->n_sides; A.F = p->F; A.n_sweeps = n_sweeps;
+        A.NR = p->NR; A.max_rows = p->max_rows;
         for (int a = 0; a < p->n_sides; ++a) {
             A.side[a] = p->side[a]; A.fam_base[a] = p->fam_base[a]; A.c[a] = p->c[a]; A.sqrt_c[a] = p->sqrt_c[a];
         }
         A.tag_base = p->tag_base;
         A.timeout_ns = p->timeout_ns;
+#ifdef SMRE_ST_KO
+        A.ko = getenv("SMRE_ST_KO") ? atoi(getenv("SMRE_ST_KO")) : 0;
+#endif
         p->tag_base += (unsigned)total;
         void *args[] = {&A};
         e = cudaLaunchCooperativeKernel(p->kernel, dim3((unsigned)(nf * p->NS)), dim3((unsigned)p->threads), args,

@@ -1,48 +1,46 @@
 // Geometry and interface of the "strips" sweep scheduler (kernel and launch in smre_strips.cu).
 // See DESIGN.md sec. 6.2.  Everything here is closed form: no tables, nothing depends on n_sweeps.
 //
-// A frame is cut into NS horizontal strips, one persistent CTA per strip; the strip keeps its rows of x in
-// shared memory for the whole call.  At a family step (s, oy, ox) (windows of one family are
-// disjoint) strip boundary j sits on the window-row grid of that family: it is the smallest grid line
-//        b_j(s, oy) = oy + s*k  >=  j*ST_T - ST_C          (b_0 = 0, b_NS = H, clipped to H),
-// so every window row ("band" of s image rows) lies inside exactly one strip, a boundary never leaves the
-// s <= ST_T rows [j*T - C, j*T - C + s), and a row that changes owner always goes to a NEIGHBOURING strip.
-// While ox runs through 0..s-1 (a "macro step" = the s families (s, oy, *)) the boundaries rest and strips do
-// not interact at all; between macro steps each boundary moves by at most s - 1 rows, up or down.
+// A frame is cut into NS horizontal strips of nominal height T, one persistent CTA per strip; the strip keeps its
+// rows of x in shared memory for the whole call.  At a family step (s, oy, ox) (windows of one family
+// are disjoint) strip boundary j sits on the window-row grid of that family: it is the smallest grid line
+//        b_j(s, oy) = oy + s*k  >=  j*T - T/2          (b_0 = 0, b_NS = H, clipped to H),
+// so every window row ("band" of s image rows) lies inside exactly one strip and a boundary never leaves the
+// s rows [j*T - T/2, j*T - T/2 + s).  While ox runs through 0..s-1 (a "macro step" = the s families (s, oy, *))
+// the boundaries rest and strips do not interact at all; between macro steps each boundary moves by at most
+// s - 1 rows, up or down, and the rows that change owner go to a strip at most ST_HOPS away.
 // Along x the bands of a strip are cut into chunks of floor(32/s) windows, one warp each, lane = column.
 #pragma once
 #include "smre_common.cuh"
 
 namespace smre {
 
-constexpr int ST_T = 8;                                   // nominal strip height (rows)
 constexpr int ST_MAX_SIDE = 8;                            // largest window side the strip kernel is compiled for
 constexpr int ST_MAX_SIDES = 8;                           // entries of sides[]
-constexpr int ST_C = 4;                                   // boundary j ranges over [j*T - C, j*T - C + s)
-constexpr int ST_SLOT_OFF = ST_C;                         // tile row of image row y in strip j: y - j*ST_T + ST_SLOT_OFF
-constexpr int ST_TR = ST_T + ST_MAX_SIDE;                 // tile rows: a strip only ever holds rows in [j*T - C, j*T - C + T + s - 1)
-constexpr int ST_MAXROWS = ST_T + ST_MAX_SIDE - 1;        // most active rows of a strip in one family step
-constexpr int ST_RU = 8;                                  // mailbox ring depth (transitions), rows moving up
-constexpr int ST_RD = 8;                                  // mailbox ring depth (transitions), rows moving down
-constexpr int ST_MAX_WARPS = 30;                          // compute warps per CTA (+ one q loader warp)
-constexpr int ST_NSTG = 32;                               // q stages (mbarrier pairs) in flight at most
+constexpr int ST_HOPS = 3;                                // a row that changes owner moves at most this many strips
+constexpr int ST_RING = 4;                                // mailbox ring depth (transitions)
+constexpr int ST_MAX_WARPS = 30;                          // compute warps per CTA (+ the waiter and the issuer warp)
+constexpr int ST_NSTG = 32;                               // q stages (mbarriers) in flight at most
+
+// rows of x a strip keeps in shared memory: it only ever holds image rows in [j*T - T/2, j*T - T/2 + T + s - 1)
+__host__ __device__ __forceinline__ int st_tile_rows(int T) { return T + ST_MAX_SIDE; }
 
 // Row at which strip j begins while the families (s, oy, *) run.
-__host__ __device__ __forceinline__ int st_boundary(int j, int NS, int H, int s, int oy)
+__host__ __device__ __forceinline__ int st_boundary(int j, int NS, int H, int T, int s, int oy)
 {
     if (j <= 0) return 0;
     if (j >= NS) return H;
-    const int d = j * ST_T - ST_C - oy;
+    const int d = j * T - T / 2 - oy;
     const int b = oy + (d > 0 ? ((d + s - 1) / s) * s : 0);
     return b < H ? b : H;
 }
 
 // Active rows [lo, hi) of strip j in family (s, oy, *): whole window rows only (reading A6: windows fully inside).
-__host__ __device__ __forceinline__ void st_active_rows(int j, int NS, int H, int s, int oy, int &lo, int &hi)
+__host__ __device__ __forceinline__ void st_active_rows(int j, int NS, int H, int T, int s, int oy, int &lo, int &hi)
 {
-    lo = st_boundary(j, NS, H, s, oy);
+    lo = st_boundary(j, NS, H, T, s, oy);
     if (lo < oy) lo = oy;
-    hi = st_boundary(j + 1, NS, H, s, oy);
+    hi = st_boundary(j + 1, NS, H, T, s, oy);
     const int ae = oy + ((H - oy) / s) * s;
     if (hi > ae) hi = ae;
     if (hi < lo) hi = lo;
@@ -53,7 +51,7 @@ __host__ __device__ __forceinline__ int st_chunk_width(int s) { return (32 / s) 
 struct StripPlan;      // host object: workspace + launch parameters
 
 struct StripSummary {
-    int strips, warps, max_rows, max_up, max_down, ring_rows, frames_per_launch;
+    int T, strips, warps, max_rows, max_hop, ring_rows, frames_per_launch;
     long long workspace_bytes;
 };
 
