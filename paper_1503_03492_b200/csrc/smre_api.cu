@@ -55,6 +55,7 @@ struct smre_handle_s {
     cudaGraphExec_t sweep_graph = nullptr;
     ConveyorPlan *plan = nullptr;      // null if the conveyor cannot tile this problem
     StripPlan *strips = nullptr;       // null if the strip kernel does not take this problem
+    char strips_why[200] = "";         // ... and why
     // incomplete
     int K = 0;
     IcdLevels levels{};
@@ -141,8 +142,8 @@ extern "C" smre_status smre_create(smre_handle *out, int H, int W, int batch, co
         e = cudaMemset(h->q, 0, h->q_bytes);
         if (e != cudaSuccess) { smre_status s2 = cuda_fail(e, "zeroing increment planes"); smre_destroy(h); return s2; }
         h->plan = conveyor_plan_create(H, W, batch, h->fams, h->q, h->xwork);     // may be null
-        char why[200] = "";
-        h->strips = strips_plan_create(H, W, batch, h->Wq, sides, c_table, n_sides, h->q, why, sizeof why);   // may be null
+        h->strips = strips_plan_create(H, W, batch, h->Wq, sides, c_table, n_sides, h->q, h->strips_why,
+                                       sizeof h->strips_why);                                              // may be null
     } else {
         int K = 0;
         while ((2 << K) <= smax) ++K;
@@ -192,7 +193,7 @@ extern "C" smre_status smre_set_schedule(smre_handle h, smre_schedule schedule)
         schedule != SMRE_SCHED_STRIPS)
         return fail(SMRE_EUNSUPPORTED, "unknown schedule %d", (int)schedule);
     if (schedule == SMRE_SCHED_STRIPS && (h->variant != SMRE_STANDARD || !h->strips))
-        return fail(SMRE_EUNSUPPORTED, "strip schedule unavailable for this handle");
+        return fail(SMRE_EUNSUPPORTED, "strip schedule unavailable for this handle: %s", h->strips_why);
     if (schedule == SMRE_SCHED_PERSISTENT && (h->variant != SMRE_STANDARD || !h->plan))
         return fail(SMRE_EUNSUPPORTED, "persistent schedule unavailable for this handle "
                                        "(incomplete variant, or tiles do not fit on chip)");

@@ -41,6 +41,7 @@ struct StripArgs {
     int side[ST_MAX_SIDES], fam_base[ST_MAX_SIDES];
     float c[ST_MAX_SIDES], sqrt_c[ST_MAX_SIDES];
     unsigned tag_base;
+    int elim;                       // 1: stores that would not change memory are not issued
     unsigned long long timeout_ns;
 #ifdef SMRE_ST_KO
     int ko;                         // timing experiments only (wrong results): parts of the kernel switched off
@@ -210,20 +211,22 @@ __device__ __forceinline__ unsigned long long pack_word(unsigned tag, float v)
     return ((unsigned long long)tag << 32) | (unsigned long long)__float_as_uint(v);
 }
 
-// In the LAST family of a macro step (sm != 0) the rows that change owner afterwards leave straight from the
-// registers: sm holds 4 bits per row of the group (see MacroEntry::sendmap), mb points at the lane's column of the
-// group's first row in the slot of the coming transition in MY mailbox (strip j + d: + d * dest_step).
+// ELIM: a store that would not change memory is not issued ("silent store elimination"): x is written back only
+// where the window was scaled or the pixel carried an increment, q only where the old or the new increment is
+// non-zero.  Memory ends up bit-identical; the q planes are still READ densely.  In the first sweep (!HAS_Q) the
+// old increments are unknown (the planes hold the previous call's), so every q is written.
 template <int S, int G, bool HAS_Q, int PITCH>
 __device__ __forceinline__ void band_group(float *xt, const float *qs, float *qg, int pitch_rt, int nvalid, bool on,
-                                           int src, float cth, float sq, int ko, unsigned long long sm,
-                                           unsigned long long *mb, long long dest_step, unsigned tag)
+                                           int src, float cth, float sq, int ko, bool elim)
 {
     const int pitch = PITCH ? PITCH : pitch_rt;
     float v[G][S], n2[G], al[G];
+    unsigned qnz[G];                                            // bit r: the pixel of row r carried an increment
 #pragma unroll
     for (int i = 0; i < G; ++i) {
         const bool pb = i == 0 || i < nvalid;
         n2[i] = 0.0f;
+        qnz[i] = 0u;
 #pragma unroll
         for (int r = 0; r < S; ++r) {
             float xv = 0.0f, qv = 0.0f;
@@ -231,6 +234,7 @@ __device__ __forceinline__ void band_group(float *xt, const float *qs, float *qg
                 xv = xt[(i * S + r) * pitch];
                 if (HAS_Q) qv = qs[(i * S + r) * pitch];
             }
+            if (HAS_Q && qv != 0.0f) qnz[i] |= 1u << r;
             v[i][r] = HAS_Q ? __fadd_rn(xv, qv) : xv;
             n2[i] = fmaf(v[i][r], v[i][r], n2[i]);
         }
@@ -240,17 +244,14 @@ __device__ __forceinline__ void band_group(float *xt, const float *qs, float *qg
 #pragma unroll
     for (int i = 0; i < G; ++i) {
         if (on && (i == 0 || i < nvalid)) {
+            const bool scaled = al[i] != 1.0f;
 #pragma unroll
             for (int r = 0; r < S; ++r) {
                 float xn, qn;
                 ball_update(v[i][r], al[i], xn, qn);
-                xt[(i * S + r) * pitch] = xn;
-                if (!(ko & 4)) __stcs(qg + (i * S + r) * pitch, qn);
-                if (sm != 0) {
-                    const int code = (int)(sm >> (4 * (i * S + r))) & 15;
-                    if (code) st_relaxed_gpu64(mb + (long long)(code - 4 + (code >= 4)) * dest_step + (i * S + r) * pitch,
-                                               pack_word(tag, xn));
-                }
+                const bool had_q = (qnz[i] >> r) & 1u;
+                if (!elim || scaled || had_q) xt[(i * S + r) * pitch] = xn;
+                if (!(ko & 4) && (!elim || !HAS_Q || had_q || qn != 0.0f)) __stcs(qg + (i * S + r) * pitch, qn);
             }
         }
     }
@@ -338,17 +339,14 @@ __device__ __forceinline__ void transition(const StripArgs &A, float *tile, int 
     const unsigned s_m3 = ld_relaxed_gpu32(A.done + (size_t)(cta - up3) * 32);
     const unsigned s_p3 = ld_relaxed_gpu32(A.done + (size_t)(cta + dn3) * 32);
 
-    // departures the last family did not make: whole rows outside the active rows, and my column of the active
-    // rows if it lay outside that family's windows
-    const int act_lo = e.lo, act_hi = e.lo + e.rows;
-    const bool idle_col = tid < e.s - 1 || tid >= e.ae_last;
+    // departures
     auto send = [&](int d, int lo, int hi, unsigned &seen) {
         if (lo >= hi) return;
         st_ring_space(A, cta, d, tag, mc, seen, w);
         if (!mine) return;
         unsigned long long *dst = box + d * dest_step;
         for (int y = lo; y < hi; ++y)
-            if (idle_col || y < act_lo || y >= act_hi) st_relaxed_gpu64(dst + y * Wq, pack_word(tag, tcol[y * pitch]));
+            st_relaxed_gpu64(dst + y * Wq, pack_word(tag, tcol[y * pitch]));
     };
     send(-1, e.send_lo[2], e.send_hi[2], cs.seen_m1);
     send(+1, e.send_lo[3], e.send_hi[3], cs.seen_p1);
@@ -433,31 +431,16 @@ __device__ __forceinline__ void macro_steps(const StripArgs &A, const MacroEntry
     float *qg = A.q + e.qoff + col0;
     const size_t q_step = (size_t)A.Btot * A.H * pitch + 1;    // next family's plane, next column
     const float *qcol = ring + col0;
-    const unsigned long long sendmap = (handoff && !ST_KO(A, 1)) ? e.sendmap : 0ull;
-    const unsigned tag_next = A.tag_base + cs.mc + 1;
-    const long long dest_step = st_dest_step(A);
+    const bool elim = A.elim != 0;
 #pragma unroll 1
     for (int ox = 0; ox < S; ++ox) {
         const bool on = w_end <= W;                            // the window lies inside the image (reading A6)
         const float *qs = HAS_Q ? qcol + ring_place(cs.pos, rows, NR) * pitch : nullptr;
-        unsigned long long sm = 0;
-        unsigned long long *mb = nullptr;
-        if (ox == S - 1 && sendmap != 0) {                     // last family: departing rows leave from the registers
-            sm = sendmap;
-            mb = st_mailbox(A, cta, j, cs.mc + 1) + (long long)e.lo * pitch + (col0 + ox);
-            if (e.send_lo[2] < e.send_hi[2]) st_ring_space(A, cta, -1, tag_next, cs.mc + 1, cs.seen_m1, w);
-            if (e.send_lo[3] < e.send_hi[3]) st_ring_space(A, cta, +1, tag_next, cs.mc + 1, cs.seen_p1, w);
-            if (e.send_lo[1] < e.send_hi[1]) st_ring_space(A, cta, -2, tag_next, cs.mc + 1, cs.seen_m2, w);
-            if (e.send_lo[4] < e.send_hi[4]) st_ring_space(A, cta, +2, tag_next, cs.mc + 1, cs.seen_p2, w);
-            if (e.send_lo[0] < e.send_hi[0]) st_ring_space(A, cta, -3, tag_next, cs.mc + 1, cs.seen_m3, w);
-            if (e.send_lo[5] < e.send_hi[5]) st_ring_space(A, cta, +3, tag_next, cs.mc + 1, cs.seen_p3, w);
-        }
         if (!(ko & 8)) {
-            band_group<S, G, HAS_Q, PITCH>(xt, qs, qg, pitch, nb, on, src, cth, sq, ko, sm, mb, dest_step, tag_next);
+            band_group<S, G, HAS_Q, PITCH>(xt, qs, qg, pitch, nb, on, src, cth, sq, ko, elim);
             for (int b0 = G; b0 < nb; b0 += G)                 // strips taller than one group
                 band_group<S, G, HAS_Q, PITCH>(xt + b0 * S * pitch, HAS_Q ? qs + b0 * S * pitch : nullptr,
-                                               qg + b0 * S * pitch, pitch, nb - b0, on, src, cth, sq, ko,
-                                               sm >> (4 * b0 * S), mb + b0 * S * pitch, dest_step, tag_next);
+                                               qg + b0 * S * pitch, pitch, nb - b0, on, src, cth, sq, ko, elim);
         }
         ++w_end;
         ++xt;
@@ -658,9 +641,8 @@ __device__ void issuer_warp(const StripArgs &A, const MacroEntry *tab, int M, fl
 }
 
 // ------------------------------------------------------------------------------------------------ kernel
-// MAXT = 672: 21 warps x 88 registers (96 do not fit); MAXT = 1024: 64 registers
 template <int PITCH, int MAXT>
-__global__ void __maxnreg__(MAXT <= 672 ? 88 : 64) strips_kernel(const __grid_constant__ StripArgs A)
+__global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__ StripArgs A)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int pitch = PITCH ? PITCH : A.Wq;
@@ -795,6 +777,7 @@ struct StripPlan {
     size_t mail_bytes = 0, smem_bytes = 0;
     unsigned tag_base = 1;
     unsigned long long timeout_ns = 2000000000ull;
+    int elim = 1;
     int device = 0;
     const void *kernel = nullptr;
     int threads = 0;
@@ -933,6 +916,7 @@ StripPlan *strips_plan_create(int H, int W, int B, int Wq, const int *sides, con
     if (Wq == 512) p->kernel = big ? kernel_ptr<512, 1024>() : kernel_ptr<512, 672>();
     else p->kernel = big ? kernel_ptr<0, 1024>() : kernel_ptr<0, 672>();
     p->smem_bytes = (size_t)st_tile_rows(p->T) * Wq * 4 + (size_t)p->NR * Wq * 4 + strips_fixed_smem();
+    if (const char *e = getenv("SMRE_DENSE_STORES")) p->elim = atoi(e) ? 0 : 1;
     if (const char *e = getenv("SMRE_TIMEOUT_MS")) {
         const long long ms = atoll(e);
         if (ms > 0) p->timeout_ns = (unsigned long long)ms * 1000000ull;
@@ -1008,6 +992,7 @@ cudaError_t strips_run(StripPlan *p, const float *y, float *x_out, int n_sweeps,
         }
         A.tag_base = p->tag_base;
         A.timeout_ns = p->timeout_ns;
+        A.elim = p->elim;
 #ifdef SMRE_ST_KO
         A.ko = getenv("SMRE_ST_KO") ? atoi(getenv("SMRE_ST_KO")) : 0;
 #endif
