@@ -101,8 +101,8 @@ extern "C" smre_status smre_create(smre_handle *out, int H, int W, int batch, co
     for (int a = 0; a < n_sides; ++a) {
         if (sides[a] < 1 || sides[a] > H || sides[a] > W)
             return fail(SMRE_EINVAL, "side %d outside [1, min(H,W)]", sides[a]);
-        if (!(c_table[a] > 0.0f) || !std::isfinite(c_table[a]))
-            return fail(SMRE_EINVAL, "threshold of side %d must be positive and finite", sides[a]);
+        if (!(c_table[a] >= 1.17549435e-38f) || !std::isfinite(c_table[a]))     // FLT_MIN: rsqrt.approx.ftz
+            return fail(SMRE_EINVAL, "threshold of side %d must be a normal positive float", sides[a]);
         for (int b = 0; b < a; ++b)
             if (sides[b] == sides[a]) return fail(SMRE_EINVAL, "duplicate side %d", sides[a]);
         if (sides[a] > smax) smax = sides[a];
@@ -222,24 +222,30 @@ extern "C" smre_status smre_project(smre_handle h, const float *y_dev, float *x_
         return SMRE_OK;
     }
 
+    // A wait of the previous strip-scheduled run on this handle that timed out (the kernel's last CTA writes the
+    // health word to pinned host memory; reading it costs nothing and needs no synchronisation)
+    if (h->strips && h->last_schedule == SMRE_SCHED_STRIPS && strips_plan_status(h->strips) != 0)
+        return fail(SMRE_ECUDA, "the previous smre_project on this handle failed: a wait of the strip scheduler timed "
+                                "out (code 0x%x), its result is invalid", strips_plan_status(h->strips));
+    // SMRE_SCHED_AUTO: the strips where they take the problem (no host planning, nothing depends on n_sweeps), else
+    // the conveyor where it can tile it, else one kernel per family
     if (h->strips && (h->schedule == SMRE_SCHED_STRIPS || h->schedule == SMRE_SCHED_AUTO)) {
-        const float *src = y_dev;
-        if (y_dev == x_out_dev) { /* in place is safe: a CTA writes rows only after their first owner has read them */ }
-        cudaError_t e = strips_run(h->strips, src, x_out_dev, n_sweeps, st, &h->last_launches);
+        // in place is safe: a CTA writes a row only after the row's first owner has read it
+        cudaError_t e = strips_run(h->strips, y_dev, x_out_dev, n_sweeps, st, &h->last_launches);
         if (e == cudaSuccess) { h->last_schedule = SMRE_SCHED_STRIPS; return SMRE_OK; }
         if (h->schedule == SMRE_SCHED_STRIPS) return cuda_fail(e, "strips_run");
-        cudaGetLastError();
+        cudaGetLastError();                        // SMRE_SCHED_AUTO: any failure to launch falls through
         h->last_launches = 0;
     }
-    const bool persistent = h->plan && (h->schedule == SMRE_SCHED_PERSISTENT ||
-                                        h->schedule == SMRE_SCHED_AUTO);
-    if (persistent) {
+    if (h->plan && (h->schedule == SMRE_SCHED_PERSISTENT || h->schedule == SMRE_SCHED_AUTO)) {
         cudaError_t e = conveyor_run(h->plan, y_dev, x_out_dev, n_sweeps, st, &h->last_launches);
         if (e == cudaSuccess) { h->last_schedule = SMRE_SCHED_PERSISTENT; return SMRE_OK; }
-        if (e != cudaErrorNotSupported) return cuda_fail(e, "conveyor_run");
-        if (h->schedule == SMRE_SCHED_PERSISTENT)
+        if (h->schedule == SMRE_SCHED_PERSISTENT) {
+            if (e != cudaErrorNotSupported) return cuda_fail(e, "conveyor_run");
             return fail(SMRE_EUNSUPPORTED, "the conveyor cannot tile %d sweeps of this problem", n_sweeps);
-        h->last_launches = 0;                      // SMRE_SCHED_AUTO: fall through to the graph schedule
+        }
+        cudaGetLastError();
+        h->last_launches = 0;
     }
     // graph schedule: x <- y, q <- 0 (Alg. 2: q_{0,s} = 0), then n_sweeps replays of the sweep graph
     h->last_schedule = SMRE_SCHED_GRAPH;
@@ -267,6 +273,11 @@ extern "C" smre_status smre_project_host(smre_handle h, const float *y_host, flo
     if (s != SMRE_OK) return s;
     CU(cudaMemcpyAsync(x_out_host, h->stage_out, bytes, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    // the stream has drained: a hand-off of a persistent scheduler that timed out must not pass as a result
+    if (h->last_schedule == SMRE_SCHED_STRIPS && h->strips && strips_plan_status(h->strips) != 0)
+        return fail(SMRE_ECUDA, "strip scheduler: a wait timed out, code 0x%x (result invalid)", strips_plan_status(h->strips));
+    if (h->last_schedule == SMRE_SCHED_PERSISTENT && h->plan && conveyor_plan_status(h->plan) != 0)
+        return fail(SMRE_ECUDA, "conveyor scheduler: a neighbour hand-off timed out (result invalid)");
     return SMRE_OK;
 }
 

@@ -267,14 +267,14 @@ __device__ __forceinline__ void project_item(float *xs, const float *qs0, float 
             v[rr] = 0.0f;
             if (k < nwin) {
                 const float xv = xs[(xi0 + rr * CV_PW) & (CV_PW * CV_PW - 1)];
-                v[rr] = first_sweep ? xv : xv + qs0[rr * qp];
+                v[rr] = first_sweep ? xv : __fadd_rn(xv, qs0[rr * qp]);
             }
             part[k] = fmaf(v[rr], v[rr], part[k]);
         }
     }
     if (part[0] >= 0.0f) CV_CLK(3);
 #pragma unroll
-    for (int m = G / 2; m > 0; m >>= 1)
+    for (int m = 1; m < G; m <<= 1)                           // neighbouring columns first, as in family_pass_kernel
 #pragma unroll
         for (int k = 0; k < KR; ++k) part[k] += __shfl_xor_sync(0xffffffffu, part[k], m);
     if (part[0] >= 0.0f) CV_CLK(4);
@@ -286,9 +286,10 @@ __device__ __forceinline__ void project_item(float *xs, const float *qs0, float 
         for (int r = 0; r < S; ++r) {
             const int rr = k * S + r;
             if (k < nwin) {
-                const float xn = alpha * v[rr];
+                float xn, qn;
+                ball_update(v[rr], alpha, xn, qn);
                 xs[(xi0 + rr * CV_PW) & (CV_PW * CV_PW - 1)] = xn;
-                __stcs(qg + rr * Wq, v[rr] - xn);
+                __stcs(qg + rr * Wq, qn);
             }
         }
     }
@@ -321,19 +322,20 @@ __device__ __forceinline__ void project_generic(Smem &sm, const GeomDesc &ge, in
                 v[r] = 0.0f;
                 if (r < s && act) {
                     const float xv = sm.xs[(xi0 + r * CV_PW) & (CV_PW * CV_PW - 1)];
-                    v[r] = first_sweep ? xv : xv + qs0[r * qp];
+                    v[r] = first_sweep ? xv : __fadd_rn(xv, qs0[r * qp]);
                 }
                 part = fmaf(v[r], v[r], part);
             }
 #pragma unroll
-            for (int m = G / 2; m > 0; m >>= 1) part += __shfl_xor_sync(0xffffffffu, part, m);
+            for (int m = 1; m < G; m <<= 1) part += __shfl_xor_sync(0xffffffffu, part, m);
             const float alpha = ball_scale(part, c, sqrt_c);
 #pragma unroll
             for (int r = 0; r < G; ++r) {
                 if (r < s && act) {
-                    const float xn = alpha * v[r];
+                    float xn, qn;
+                    ball_update(v[r], alpha, xn, qn);
                     sm.xs[(xi0 + r * CV_PW) & (CV_PW * CV_PW - 1)] = xn;
-                    __stcs(qg + r * Wq, v[r] - xn);
+                    __stcs(qg + r * Wq, qn);
                 }
             }
         }
@@ -755,6 +757,10 @@ conveyor_kernel(const __grid_constant__ CParams p)
                         }
                     }
                     if (k > 0) {
+                        // single tile: the q rows of this box were written by this CTA's compute warps with generic-proxy
+                        // stores one sweep ago; the step barriers order them before this point at CTA scope, the fence
+                        // orders the async-proxy read of the TMA behind them (the multi-tile path fences above)
+                        if (!ordered) asm volatile("fence.proxy.async.global;" ::: "memory");
                         mbar_expect_tx(&sm.qbar[stp], (unsigned)(k * 8 * p.qp * 4));
                         tma_load_2d_hint(sm.qs + (size_t)stp * (CV_PW * CV_PW), &p.qmap[k - 1], d.tma_col, d.tma_row, &sm.qbar[stp], q_policy);
                     }
@@ -1223,8 +1229,10 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
     memcpy(p.qmap, pl->qmap, sizeof p.qmap);
     const int tiles = pl->NR * pl->NC;
     if ((e = cudaMemsetAsync(pl->d_status, 0, sizeof(int), st)) != cudaSuccess) return e;   // health flag of THIS run
-    const char *trace_path = getenv("SMRE_CV_TRACE");        // debug only: synchronises and writes a file
+#ifdef SMRE_CV_TRACE_BUILD                                  // debug builds only: synchronises and writes a file
+    const char *trace_path = getenv("SMRE_CV_TRACE");
     if (trace_path && cudaMalloc(&p.trace, (size_t)tiles * p.total * 64) != cudaSuccess) p.trace = nullptr;
+#endif
     for (int f0 = 0; f0 < pl->B; f0 += pl->frames_per_launch) {
         p.frame0 = f0;
         const int nb = std::min(pl->frames_per_launch, pl->B - f0);
@@ -1237,6 +1245,7 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
         if (e != cudaSuccess) return e;
         if (launches) ++*launches;
     }
+#ifdef SMRE_CV_TRACE_BUILD
     if (p.trace) {
         std::vector<unsigned long long> t((size_t)tiles * p.total * 8);
         cudaStreamSynchronize(st);
@@ -1249,6 +1258,7 @@ cudaError_t conveyor_run(ConveyorPlan *pl, const float *y, float *x_out, int n_s
             fclose(fh);
         }
     }
+#endif
     return cudaSuccess;
 }
 
