@@ -22,7 +22,9 @@
  * x + sum_f q_f == y, feasibility in the limit, variational inequality, KKT
  * structure, SLSQP brute force on tiny images, box-cap-ball closed form,
  * symmetries, ICD == composition of restricted standard runs == explicit
- * tile-by-tile solve, counts.  No function here is "parity unpinned".
+ * tile-by-tile solve, counts, the all-windows checker against a strided-view
+ * sum, the stop rules of the tolerance modes against fixed-count runs and an
+ * independent tile-wise solve.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdlib.h>
@@ -244,4 +246,135 @@ int smre_oracle_window_sums(const double *x, int H, int W, int s, double *out)
             out[(size_t)wy * nwx + wx] = n2;
         }
     return 0;
+}
+
+/* ===========================================================================
+ * Convergence-controlled runs: the paper never runs a
+ * fixed sweep count.
+ *
+ * Standard variant, Alg. 2: "while ||x_r - x_{r-1}||_2^2 >
+ * delta".  Reading A4': r counts SWEEPS (one pass over all families, reading
+ * A2), x_r is the image after sweep r, x_0 = y; the run stops after the first
+ * sweep r >= 1 with ||x_r - x_{r-1}||^2 <= delta, or after max_sweeps.
+ * *sweeps_done receives r.  The square sum runs row-major over the image.
+ * ------------------------------------------------------------------------- */
+int smre_oracle_std_tol(const double *y, int H, int W, const int *sides, const double *c,
+                        int n_sides, int max_sweeps, double delta, double *x_out,
+                        int *sweeps_done)
+{
+    if (!y || !x_out || !sides || !c || n_sides <= 0 || H <= 0 || W <= 0 || max_sweeps < 1)
+        return -1;
+    int F = smre_oracle_std_family_count(sides, n_sides);
+    size_t N = (size_t)H * W;
+    int *fs = (int *)malloc(sizeof(int) * 3 * (size_t)F);
+    double *fc = (double *)malloc(sizeof(double) * (size_t)F);
+    double *q = (double *)calloc(N * (size_t)F, sizeof(double));
+    double *prev = (double *)malloc(sizeof(double) * N);
+    if (!fs || !fc || !q || !prev) { free(fs); free(fc); free(q); free(prev); return -1; }
+    smre_oracle_std_family_list(sides, c, n_sides, fs, fs + F, fs + 2 * F, fc);
+    if (x_out != y) memcpy(x_out, y, sizeof(double) * N);
+    int r = 0;
+    for (;;) {
+        memcpy(prev, x_out, sizeof(double) * N);                 /* x_{r-1} */
+        for (int f = 0; f < F; ++f)
+            family_pass(x_out, q + (size_t)f * N, H, W, fs[f], fs[F + f], fs[2 * F + f], fc[f]);
+        ++r;
+        double d2 = 0.0;
+        for (size_t i = 0; i < N; ++i) {
+            double d = x_out[i] - prev[i];
+            d2 += d * d;
+        }
+        if (!(d2 > delta) || r >= max_sweeps) break;             /* while ||x_r - x_{r-1}||^2 > delta */
+    }
+    if (sweeps_done) *sweeps_done = r;
+    free(fs); free(fc); free(q); free(prev);
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * Incomplete variant with the stop rule of Listing 3:
+ * every thread block iterates ITS tile "while (delta > tol*1024)", where delta
+ * collects mabs(e_old - e_new) of the block's pixels over all levels of one
+ * cycle and 1024 is the number of pixels of the paper's 32 x 32 tile.
+ * Readings (DESIGN.md A-ICD-16): the tile is the L x L square, L = 2^K, of the
+ * tiling with origin (2^i mod L) on the diagonal (virtual tiles overhang the
+ * border, A-ICD-13); delta = sum over the levels K..i of one cycle and over the
+ * tile's pixels inside the image of |x_old - x_new| (the block-wide reduction
+ * the listing elides, A-ICD-11); a tile stops after the first cycle with
+ * delta <= tol * L^2, or after max_cycles.  Tiles are independent (all windows
+ * of a shift nest inside its tiles), so this is tile-serial.
+ *   cycles_total : NULL or sum over shifts and tiles of the cycles run
+ *   cycles_max   : NULL or the largest cycle count of any tile
+ * ------------------------------------------------------------------------- */
+int smre_oracle_icd_levels_tol(const double *y, int H, int W, int K, const double *level_c,
+                               int max_cycles, double tol, double *x_out,
+                               long long *cycles_total, int *cycles_max)
+{
+    if (!y || !x_out || !level_c || H <= 0 || W <= 0 || K < 0 || K > 12 || max_cycles < 1)
+        return -1;
+    const int L = 1 << K;
+    size_t N = (size_t)H * W;
+    double *q = (double *)malloc(sizeof(double) * N * (size_t)(K + 1));
+    double *tmp = (double *)malloc(sizeof(double) * (size_t)L * L);
+    if (!q || !tmp) { free(q); free(tmp); return -1; }
+    if (x_out != y) memcpy(x_out, y, sizeof(double) * N);
+    long long total = 0;
+    int cmax = 0;
+    for (int i = 0; i <= K; ++i) {                                /* shift loop, Listing 2 */
+        const int shift = 1 << i, o = shift % L;
+        memset(q, 0, sizeof(double) * N * (size_t)(K + 1));       /* "Set q = 0" */
+        for (int ty = o - L; ty < H; ty += L)                     /* tiles of this shift, incl. overhanging ones */
+            for (int tx = o - L; tx < W; tx += L) {
+                if (ty + L <= 0 || tx + L <= 0) continue;
+                int cyc = 0;
+                for (;;) {
+                    double delta = 0.0;
+                    for (int k = K; k >= i; --k) {                /* for (s = 5; s >= smin; s--) */
+                        const int side = 1 << k;
+                        double *qk = q + (size_t)k * N;
+                        for (int wy = ty; wy < ty + L; wy += side)
+                            for (int wx = tx; wx < tx + L; wx += side) {
+                                if (wy < 0 || wx < 0 || wy + side > H || wx + side > W) continue;
+                                /* keep the old values, take the step, add |e_old - e_new| */
+                                for (int r = 0; r < side; ++r)
+                                    for (int cc = 0; cc < side; ++cc)
+                                        tmp[r * side + cc] = x_out[(size_t)(wy + r) * W + wx + cc];
+                                window_step(x_out, qk, W, wy, wx, side, level_c[k]);
+                                for (int r = 0; r < side; ++r)
+                                    for (int cc = 0; cc < side; ++cc)
+                                        delta += fabs(tmp[r * side + cc] - x_out[(size_t)(wy + r) * W + wx + cc]);
+                            }
+                    }
+                    ++cyc;
+                    if (!(delta > tol * (double)L * (double)L) || cyc >= max_cycles) break;
+                }
+                total += cyc;
+                if (cyc > cmax) cmax = cyc;
+            }
+    }
+    if (cycles_total) *cycles_total = total;
+    if (cycles_max) *cycles_max = cmax;
+    free(q);
+    free(tmp);
+    return 0;
+}
+
+int smre_oracle_icd_tol(const double *y, int H, int W, const int *sides, const double *c,
+                        int n_sides, int max_cycles, double tol, double *x_out,
+                        long long *cycles_total, int *cycles_max)
+{
+    if (!sides || !c || n_sides <= 0) return -1;
+    int smax = 0;
+    for (int a = 0; a < n_sides; ++a) if (sides[a] > smax) smax = sides[a];
+    if (smax < 1) return -1;
+    int K = 0;
+    while ((2 << K) <= smax) ++K;
+    double level_c[32];
+    for (int k = 0; k <= K; ++k) {
+        int found = 0;
+        for (int a = 0; a < n_sides; ++a)
+            if (sides[a] == (1 << k)) { level_c[k] = c[a]; found = 1; break; }
+        if (!found) return -2;
+    }
+    return smre_oracle_icd_levels_tol(y, H, W, K, level_c, max_cycles, tol, x_out, cycles_total, cycles_max);
 }

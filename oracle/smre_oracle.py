@@ -59,6 +59,14 @@ def _load():
         lib.smre_oracle_icd.restype = ctypes.c_int
         lib.smre_oracle_icd.argtypes = [
             _dp, ctypes.c_int, ctypes.c_int, _ip, _dp, ctypes.c_int, ctypes.c_int, _dp]
+        lib.smre_oracle_std_tol.restype = ctypes.c_int
+        lib.smre_oracle_std_tol.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, _ip, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+            _dp, _ip]
+        lib.smre_oracle_icd_tol.restype = ctypes.c_int
+        lib.smre_oracle_icd_tol.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, _ip, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+            _dp, ctypes.POINTER(ctypes.c_longlong), _ip]
         lib.smre_oracle_window_sums.restype = ctypes.c_int
         lib.smre_oracle_window_sums.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
         _lib = lib
@@ -158,6 +166,44 @@ def project_icd(y, sides, c, n_sweeps):
                              int(n_sweeps), _p(x, _dp))
     _check(rc, "smre_oracle_icd")
     return x
+
+
+def project_std_tol(y, sides, c, max_sweeps, delta):
+    """Alg. 2 with its stop rule ||x_r - x_{r-1}||^2 <= delta per sweep.
+    One image [H,W] -> (x, sweeps_done); a stack [B,H,W] -> (x, [sweeps_done per frame])."""
+    lib = _load()
+    y = _f64(y)
+    sides = _i32(sides)
+    c = _f64(c)
+    if y.ndim == 3:
+        res = [project_std_tol(f, sides, c, max_sweeps, delta) for f in y]
+        return np.stack([r[0] for r in res]), [r[1] for r in res]
+    H, W = y.shape
+    x = np.empty_like(y)
+    done = ctypes.c_int(0)
+    rc = lib.smre_oracle_std_tol(_p(y, _dp), H, W, _p(sides, _ip), _p(c, _dp), len(sides),
+                                 int(max_sweeps), float(delta), _p(x, _dp), ctypes.byref(done))
+    _check(rc, "smre_oracle_std_tol")
+    return x, done.value
+
+
+def project_icd_tol(y, sides, c, max_cycles, tol):
+    """Incomplete variant, every tile iterated until Listing 3's sum |delta| <= tol * L^2.
+    One image [H,W] -> (x, cycles_total, cycles_max); a stack -> (x, sum, max) over the frames."""
+    lib = _load()
+    y = _f64(y)
+    sides = _i32(sides)
+    c = _f64(c)
+    if y.ndim == 3:
+        res = [project_icd_tol(f, sides, c, max_cycles, tol) for f in y]
+        return np.stack([r[0] for r in res]), sum(r[1] for r in res), max(r[2] for r in res)
+    H, W = y.shape
+    x = np.empty_like(y)
+    tot, mx = ctypes.c_longlong(0), ctypes.c_int(0)
+    rc = lib.smre_oracle_icd_tol(_p(y, _dp), H, W, _p(sides, _ip), _p(c, _dp), len(sides),
+                                 int(max_cycles), float(tol), _p(x, _dp), ctypes.byref(tot), ctypes.byref(mx))
+    _check(rc, "smre_oracle_icd_tol")
+    return x, tot.value, mx.value
 
 
 def project(y, sides, c, n_sweeps, variant):
