@@ -139,6 +139,27 @@ smre_status smre_plan_check(int H, int W, const int *sides, int n_sides, int n_s
                             int *tiles_y, int *tiles_x, int *max_tile_h, int *max_tile_w,
                             long long *table_bytes);
 
+/* ---- a projection that allocates nothing ------------------------------------------------------ */
+
+/* Size of the file-scope device array that serves as the scratch of smre_project_noalloc: every GPU that loads
+ * the library holds this much device memory until the process exits. */
+#define SMRE_NOALLOC_MAX_BYTES (16 * 1024 * 1024)
+
+/*
+ * SMRE_STANDARD projection of ONE H x W image (Alg. 2; Eq. 14) for callers that
+ * cannot allocate: no handle, and no cudaMalloc, cudaFree or any other allocating routine is called.  Same
+ * arguments, family order and arithmetic as smre_create(..., SMRE_STANDARD) + smre_project under
+ * SMRE_SCHED_GRAPH (bit-identical results); one kernel launch per family and sweep, enqueued on cuda_stream,
+ * asynchronous.  y_dev / x_out_dev: DEVICE pointers to H*W fp32 (x_out_dev == y_dev allowed); sides / c_table:
+ * HOST arrays.  The increment planes, sum(side^2) * H * Wq * 4 bytes (Wq = W rounded up to a multiple of 4), live
+ * in a static device array of SMRE_NOALLOC_MAX_BYTES on the CURRENT device: a larger problem is refused with
+ * SMRE_EUNSUPPORTED (64 x 64 with sides 1-4 needs 480 KiB; 256 x 256 with sides 1-4 7.5 MiB).
+ * The array is shared by all calls and keeps the last call's contents; each call zeroes what it uses first.
+ * Calls that overlap on the GPU (other streams, other threads) RACE on it: serialise them.
+ */
+smre_status smre_project_noalloc(int H, int W, const int *sides, int n_sides, const float *c_table,
+                                 const float *y_dev, float *x_out_dev, int n_sweeps, void *cuda_stream);
+
 /* Text of the last error on the calling thread ("" if none).  Never NULL. */
 const char *smre_last_error(void);
 

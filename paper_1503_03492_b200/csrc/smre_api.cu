@@ -68,6 +68,10 @@ struct smre_handle_s {
 
 extern "C" const char *smre_last_error(void) { return g_err; }
 
+namespace smre {
+void set_last_error(const char *text) { snprintf(g_err, sizeof g_err, "%s", text ? text : ""); }
+}
+
 static smre_status build_sweep_graph(smre_handle h)
 {
     cudaStream_t cs;

@@ -40,6 +40,9 @@ __device__ __forceinline__ void ball_update(float v, float alpha, float &xn, flo
     qn = __fsub_rn(v, xn);
 }
 
+// smre_api.cu: text returned by smre_last_error() on the calling thread (for entry points in other files)
+void set_last_error(const char *text);
+
 // ---- launchers implemented in the .cu files --------------------------------------------------
 
 // smre_family.cu: one family pass over all frames (schedule SMRE_SCHED_GRAPH).  x: [B][H][W];

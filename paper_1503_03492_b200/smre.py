@@ -21,7 +21,7 @@ _STATUS = {0: "SMRE_OK", 1: "SMRE_EINVAL", 2: "SMRE_EUNSUPPORTED", 3: "SMRE_ENOM
 exported_symbols = (
     "smre_create", "smre_project", "smre_project_host", "smre_destroy", "smre_set_schedule",
     "smre_info", "smre_family", "smre_export_increments", "smre_last_launch", "smre_last_error",
-    "smre_plan_check",
+    "smre_plan_check", "smre_project_noalloc",
 )
 
 
@@ -61,6 +61,7 @@ def load_library(build_if_missing: bool = True):
     lib.smre_last_launch.argtypes = [_vp, _ip, _llp, _ip, _ip]
     lib.smre_plan_check.argtypes = [ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                     _ip, _ip, _ip, _ip, _llp]
+    lib.smre_project_noalloc.argtypes = [ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, _fp, _vp, _vp, ctypes.c_int, _vp]
     for name in exported_symbols:
         getattr(lib, name).restype = ctypes.c_int
     lib.smre_last_error.restype = ctypes.c_char_p
@@ -100,6 +101,17 @@ def smre_project(handle, y_ptr, x_out_ptr, n_sweeps, stream=0):
 def smre_project_host(handle, y_ptr, x_out_ptr, n_sweeps, stream=0):
     """Host addresses (numpy .ctypes.data or pinned tensor.data_ptr()); blocks until done."""
     _check(load_library().smre_project_host(handle, y_ptr, x_out_ptr, int(n_sweeps), stream))
+
+
+def smre_project_noalloc(H, W, sides, c_table, y_ptr, x_out_ptr, n_sweeps, stream=0):
+    """Standard projection of one H x W image with the increment planes in the library's static device scratch
+    (SMRE_NOALLOC_MAX_BYTES): allocates nothing.  y_ptr / x_out_ptr: device addresses."""
+    sides = np.ascontiguousarray(sides, dtype=np.int32)
+    c_table = np.ascontiguousarray(c_table, dtype=np.float32)
+    if sides.ndim != 1 or sides.shape != c_table.shape:
+        raise ValueError("sides and c_table must be 1-D and of equal length")
+    _check(load_library().smre_project_noalloc(int(H), int(W), sides.ctypes.data_as(_ip), len(sides),
+                                               c_table.ctypes.data_as(_fp), y_ptr, x_out_ptr, int(n_sweeps), stream))
 
 
 def smre_destroy(handle):
