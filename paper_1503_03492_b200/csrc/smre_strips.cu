@@ -211,22 +211,23 @@ __device__ __forceinline__ unsigned long long pack_word(unsigned tag, float v)
     return ((unsigned long long)tag << 32) | (unsigned long long)__float_as_uint(v);
 }
 
-// ELIM: a store that would not change memory is not issued ("silent store elimination"): x is written back only
-// where the window was scaled or the pixel carried an increment, q only where the old or the new increment is
-// non-zero.  Memory ends up bit-identical; the q planes are still READ densely.  In the first sweep (!HAS_Q) the
-// old increments are unknown (the planes hold the previous call's), so every q is written.
+// ELIM: work that would not change memory is not done.  A lane's column of a window is LIVE if the window was
+// scaled (alpha != 1) or any pixel of the column carried an increment; only live columns compute and store the
+// update.  For the others x' = 1 * (x + 0) = x and q' = v - v = 0 are what memory already holds, bit for bit
+// (the planes are zeroed at create, v - v is +0).  The q planes are still READ densely.  In the first sweep
+// (!HAS_Q) the planes hold the previous call's increments, so every column is live and every q is written.
 template <int S, int G, bool HAS_Q, int PITCH>
 __device__ __forceinline__ void band_group(float *xt, const float *qs, float *qg, int pitch_rt, int nvalid, bool on,
                                            int src, float cth, float sq, int ko, bool elim)
 {
     const int pitch = PITCH ? PITCH : pitch_rt;
     float v[G][S], n2[G], al[G];
-    unsigned qnz[G];                                            // bit r: the pixel of row r carried an increment
+    unsigned qbits[G];                                          // OR of the bit patterns of the column's increments
 #pragma unroll
     for (int i = 0; i < G; ++i) {
         const bool pb = i == 0 || i < nvalid;
         n2[i] = 0.0f;
-        qnz[i] = 0u;
+        qbits[i] = 0u;
 #pragma unroll
         for (int r = 0; r < S; ++r) {
             float xv = 0.0f, qv = 0.0f;
@@ -234,7 +235,7 @@ __device__ __forceinline__ void band_group(float *xt, const float *qs, float *qg
                 xv = xt[(i * S + r) * pitch];
                 if (HAS_Q) qv = qs[(i * S + r) * pitch];
             }
-            if (HAS_Q && qv != 0.0f) qnz[i] |= 1u << r;
+            if (HAS_Q) qbits[i] |= __float_as_uint(qv);
             v[i][r] = HAS_Q ? __fadd_rn(xv, qv) : xv;
             n2[i] = fmaf(v[i][r], v[i][r], n2[i]);
         }
@@ -243,15 +244,14 @@ __device__ __forceinline__ void band_group(float *xt, const float *qs, float *qg
     for (int i = 0; i < G; ++i) al[i] = ball_scale(window_total<S>(n2[i], src), cth, sq);
 #pragma unroll
     for (int i = 0; i < G; ++i) {
-        if (on && (i == 0 || i < nvalid)) {
-            const bool scaled = al[i] != 1.0f;
+        const bool live = !elim || !HAS_Q || al[i] != 1.0f || (qbits[i] << 1) != 0u;
+        if (on && (i == 0 || i < nvalid) && live) {
 #pragma unroll
             for (int r = 0; r < S; ++r) {
                 float xn, qn;
                 ball_update(v[i][r], al[i], xn, qn);
-                const bool had_q = (qnz[i] >> r) & 1u;
-                if (!elim || scaled || had_q) xt[(i * S + r) * pitch] = xn;
-                if (!(ko & 4) && (!elim || !HAS_Q || had_q || qn != 0.0f)) __stcs(qg + (i * S + r) * pitch, qn);
+                xt[(i * S + r) * pitch] = xn;
+                if (!(ko & 4)) __stcs(qg + (i * S + r) * pitch, qn);
             }
         }
     }
