@@ -912,9 +912,9 @@ StripPlan *strips_plan_create(int H, int W, int B, int Wq, const int *sides, con
     }
     p->F = F;
     p->threads = (p->NWC + 2) * 32;                               // compute warps + waiter + issuer
-    const bool big = p->threads > 672;
-    if (Wq == 512) p->kernel = big ? kernel_ptr<512, 1024>() : kernel_ptr<512, 672>();
-    else p->kernel = big ? kernel_ptr<0, 1024>() : kernel_ptr<0, 672>();
+    const bool big = p->threads > 576;
+    if (Wq == 512) p->kernel = big ? kernel_ptr<512, 1024>() : kernel_ptr<512, 576>();
+    else p->kernel = big ? kernel_ptr<0, 1024>() : kernel_ptr<0, 576>();
     p->smem_bytes = (size_t)st_tile_rows(p->T) * Wq * 4 + (size_t)p->NR * Wq * 4 + strips_fixed_smem();
     if (const char *e = getenv("SMRE_DENSE_STORES")) p->elim = atoi(e) ? 0 : 1;
     if (const char *e = getenv("SMRE_TIMEOUT_MS")) {
