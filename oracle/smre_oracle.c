@@ -306,9 +306,59 @@ int smre_oracle_std_tol(const double *y, int H, int W, const int *sides, const d
  *   cycles_total : NULL or sum over shifts and tiles of the cycles run
  *   cycles_max   : NULL or the largest cycle count of any tile
  * ------------------------------------------------------------------------- */
+static int icd_levels_tol_impl(const double *y, int H, int W, int K, const double *level_c,
+                               int max_cycles, double tol, double *x_out,
+                               long long *cycles_total, int *cycles_max,
+                               int *tile_cycles_out, const int *tile_cycles_in, double band,
+                               long long *n_bad);
+
 int smre_oracle_icd_levels_tol(const double *y, int H, int W, int K, const double *level_c,
                                int max_cycles, double tol, double *x_out,
                                long long *cycles_total, int *cycles_max)
+{
+    return icd_levels_tol_impl(y, H, W, K, level_c, max_cycles, tol, x_out, cycles_total, cycles_max,
+                               NULL, NULL, 0.0, NULL);
+}
+
+/* Number of tiles along an axis of extent N for shift i (tile edge L): origins o - L, o, o + L, ...
+ * with o = 2^i mod L, those with origin + L <= 0 left out. */
+int smre_oracle_icd_tiles_along(int N, int K, int i)
+{
+    const int L = 1 << K, o = (1 << i) % L;
+    int n = 0;
+    for (int t = o - L; t < N; t += L)
+        if (t + L > 0) ++n;
+    return n;
+}
+
+/* Same run, additionally writing the cycles every tile ran: tile_cycles_out, shift-major, per shift
+ * [tiles along y][tiles along x] (smre_oracle_icd_tiles_along). */
+int smre_oracle_icd_levels_tol_counts(const double *y, int H, int W, int K, const double *level_c,
+                                      int max_cycles, double tol, double *x_out, int *tile_cycles_out)
+{
+    return icd_levels_tol_impl(y, H, W, K, level_c, max_cycles, tol, x_out, NULL, NULL,
+                               tile_cycles_out, NULL, 0.0, NULL);
+}
+
+/* REPLAY of somebody else's stop decisions (the fp32 kernel's): every tile runs exactly the cycles
+ * tile_cycles_in prescribes (same layout), and the fp64 deltas are checked against those decisions
+ * within a relative band: a tile that ran c cycles must have had delta > tol L^2 (1 - band) after
+ * every cycle before c, and delta <= tol L^2 (1 + band) after cycle c unless c == max_cycles.
+ * *n_bad counts the tiles whose count the band does not allow. */
+int smre_oracle_icd_levels_replay(const double *y, int H, int W, int K, const double *level_c,
+                                  int max_cycles, double tol, const int *tile_cycles_in, double band,
+                                  double *x_out, long long *n_bad)
+{
+    if (!tile_cycles_in || !n_bad) return -1;
+    return icd_levels_tol_impl(y, H, W, K, level_c, max_cycles, tol, x_out, NULL, NULL,
+                               NULL, tile_cycles_in, band, n_bad);
+}
+
+static int icd_levels_tol_impl(const double *y, int H, int W, int K, const double *level_c,
+                               int max_cycles, double tol, double *x_out,
+                               long long *cycles_total, int *cycles_max,
+                               int *tile_cycles_out, const int *tile_cycles_in, double band,
+                               long long *n_bad)
 {
     if (!y || !x_out || !level_c || H <= 0 || W <= 0 || K < 0 || K > 12 || max_cycles < 1)
         return -1;
@@ -318,15 +368,19 @@ int smre_oracle_icd_levels_tol(const double *y, int H, int W, int K, const doubl
     double *tmp = (double *)malloc(sizeof(double) * (size_t)L * L);
     if (!q || !tmp) { free(q); free(tmp); return -1; }
     if (x_out != y) memcpy(x_out, y, sizeof(double) * N);
-    long long total = 0;
+    long long total = 0, bad = 0;
+    size_t tile_idx = 0;
     int cmax = 0;
+    const double thresh = tol * (double)L * (double)L;
     for (int i = 0; i <= K; ++i) {                                /* shift loop, Listing 2 */
         const int shift = 1 << i, o = shift % L;
         memset(q, 0, sizeof(double) * N * (size_t)(K + 1));       /* "Set q = 0" */
         for (int ty = o - L; ty < H; ty += L)                     /* tiles of this shift, incl. overhanging ones */
             for (int tx = o - L; tx < W; tx += L) {
                 if (ty + L <= 0 || tx + L <= 0) continue;
-                int cyc = 0;
+                const int prescribed = tile_cycles_in ? tile_cycles_in[tile_idx] : 0;
+                int cyc = 0, tile_bad = 0;
+                if (tile_cycles_in && (prescribed < 1 || prescribed > max_cycles)) { ++bad; ++tile_idx; continue; }
                 for (;;) {
                     double delta = 0.0;
                     for (int k = K; k >= i; --k) {                /* for (s = 5; s >= smin; s--) */
@@ -346,12 +400,22 @@ int smre_oracle_icd_levels_tol(const double *y, int H, int W, int K, const doubl
                             }
                     }
                     ++cyc;
-                    if (!(delta > tol * (double)L * (double)L) || cyc >= max_cycles) break;
+                    if (tile_cycles_in) {                         /* replay: the count is given, the deltas are checked */
+                        if (cyc < prescribed) { if (!(delta > thresh * (1.0 - band))) tile_bad = 1; }
+                        else {
+                            if (cyc < max_cycles && delta > thresh * (1.0 + band)) tile_bad = 1;
+                            break;
+                        }
+                    } else if (!(delta > thresh) || cyc >= max_cycles) break;
                 }
                 total += cyc;
+                bad += tile_bad;
                 if (cyc > cmax) cmax = cyc;
+                if (tile_cycles_out) tile_cycles_out[tile_idx] = cyc;
+                ++tile_idx;
             }
     }
+    if (n_bad) *n_bad = bad;
     if (cycles_total) *cycles_total = total;
     if (cycles_max) *cycles_max = cmax;
     free(q);

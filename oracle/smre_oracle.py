@@ -67,6 +67,15 @@ def _load():
         lib.smre_oracle_icd_tol.argtypes = [
             _dp, ctypes.c_int, ctypes.c_int, _ip, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_double,
             _dp, ctypes.POINTER(ctypes.c_longlong), _ip]
+        lib.smre_oracle_icd_tiles_along.restype = ctypes.c_int
+        lib.smre_oracle_icd_tiles_along.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int]
+        lib.smre_oracle_icd_levels_tol_counts.restype = ctypes.c_int
+        lib.smre_oracle_icd_levels_tol_counts.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_int, ctypes.c_double, _dp, _ip]
+        lib.smre_oracle_icd_levels_replay.restype = ctypes.c_int
+        lib.smre_oracle_icd_levels_replay.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_int, ctypes.c_double, _ip,
+            ctypes.c_double, _dp, ctypes.POINTER(ctypes.c_longlong)]
         lib.smre_oracle_window_sums.restype = ctypes.c_int
         lib.smre_oracle_window_sums.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
         _lib = lib
@@ -204,6 +213,56 @@ def project_icd_tol(y, sides, c, max_cycles, tol):
                                  int(max_cycles), float(tol), _p(x, _dp), ctypes.byref(tot), ctypes.byref(mx))
     _check(rc, "smre_oracle_icd_tol")
     return x, tot.value, mx.value
+
+
+def _icd_levels(sides, c):
+    sides = [int(v) for v in sides]
+    K = int(np.floor(np.log2(max(sides))))
+    c_of = {s: float(v) for s, v in zip(sides, c)}
+    return K, _f64([c_of[1 << k] for k in range(K + 1)])
+
+
+def icd_tile_grid(H, W, K):
+    """[(tiles along y, tiles along x)] per shift i = 0..K: the layout of the per-tile cycle counts."""
+    lib = _load()
+    return [(lib.smre_oracle_icd_tiles_along(int(H), K, i), lib.smre_oracle_icd_tiles_along(int(W), K, i))
+            for i in range(K + 1)]
+
+
+def project_icd_tol_counts(y, sides, c, max_cycles, tol):
+    """As project_icd_tol on ONE image, returning (x, [per shift: int32 array (ty, tx) of cycles run])."""
+    lib = _load()
+    y = _f64(y)
+    H, W = y.shape
+    K, lc = _icd_levels(sides, c)
+    grid = icd_tile_grid(H, W, K)
+    counts = np.zeros(sum(a * b for a, b in grid), np.int32)
+    x = np.empty_like(y)
+    _check(lib.smre_oracle_icd_levels_tol_counts(_p(y, _dp), H, W, K, _p(lc, _dp), int(max_cycles), float(tol),
+                                                 _p(x, _dp), _p(counts, _ip)), "smre_oracle_icd_levels_tol_counts")
+    out, o = [], 0
+    for a, b in grid:
+        out.append(counts[o:o + a * b].reshape(a, b).copy())
+        o += a * b
+    return x, out
+
+
+def replay_icd(y, sides, c, max_cycles, tol, tile_cycles, band):
+    """Every tile runs exactly the cycles tile_cycles prescribes (list per shift of (ty, tx) arrays, e.g. the CUDA
+    path's); returns (x, n_bad): n_bad tiles whose count the fp64 deltas do not allow within the relative band."""
+    lib = _load()
+    y = _f64(y)
+    H, W = y.shape
+    K, lc = _icd_levels(sides, c)
+    grid = icd_tile_grid(H, W, K)
+    assert len(tile_cycles) == K + 1 and all(np.asarray(t).shape == g for t, g in zip(tile_cycles, grid))
+    counts = _i32(np.concatenate([np.asarray(t).ravel() for t in tile_cycles]))
+    x = np.empty_like(y)
+    bad = ctypes.c_longlong(0)
+    _check(lib.smre_oracle_icd_levels_replay(_p(y, _dp), H, W, K, _p(lc, _dp), int(max_cycles), float(tol),
+                                             _p(counts, _ip), float(band), _p(x, _dp), ctypes.byref(bad)),
+           "smre_oracle_icd_levels_replay")
+    return x, bad.value
 
 
 def project(y, sides, c, n_sweeps, variant):

@@ -131,3 +131,30 @@ def test_icd_tol_degenerate_cases(oracle):
     # the cycle counts do not increase with tol
     tots = [oracle.project_icd_tol(y, sides, c, 2000, t)[1] for t in (1e-6, 1e-4, 1e-2, 1.0)]
     assert all(a >= b for a, b in zip(tots, tots[1:])) and tots[0] > tots[-1]
+
+
+# ---- per-tile counts and the replay used to check the kernel's fp32 stop decisions ---------------------
+def test_icd_replay_of_own_counts_is_exact_and_detects_wrong_counts(oracle):
+    rng = np.random.default_rng(31)
+    y = 2.0 * rng.standard_normal((29, 42))
+    sides = [1, 2, 4, 8]
+    c = C(sides)
+    x, total, cmax = oracle.project_icd_tol(y, sides, c, 300, 1e-3)
+    x2, counts = oracle.project_icd_tol_counts(y, sides, c, 300, 1e-3)
+    assert np.array_equal(x, x2)
+    assert [t.shape for t in counts] == oracle.icd_tile_grid(29, 42, 3)
+    assert sum(int(t.sum()) for t in counts) == total and max(int(t.max()) for t in counts) == cmax
+    # the counts of the independent numpy tile-wise solve (same enumeration: shifts, then tile rows, then columns)
+    want, wtotal, wmax = tilewise_icd_tol(y, 3, c, 300, 1e-3)
+    assert (total, cmax) == (wtotal, wmax)
+    # replaying its own decisions reproduces the result and finds nothing to object to, even with a zero band
+    xr, bad = oracle.replay_icd(y, sides, c, 300, 1e-3, counts, 0.0)
+    assert bad == 0 and np.array_equal(xr, x)
+    # one cycle too few / too many on a tile that iterated: the deltas do not allow it
+    i, (ty, tx) = max(((i, np.unravel_index(t.argmax(), t.shape)) for i, t in enumerate(counts)),
+                      key=lambda a: counts[a[0]][a[1]])
+    for d in (-1, +1):
+        wrong = [t.copy() for t in counts]
+        wrong[i][ty, tx] += d
+        _, bad = oracle.replay_icd(y, sides, c, 300, 1e-3, wrong, 1e-6)
+        assert bad == 1
