@@ -21,7 +21,9 @@
  *                      fine) whose origin is (2^i mod side) on the diagonal; n_sweeps inner cycles
  *                      per shift.  Increments never leave the chip.
  *
- * All arithmetic is fp32, IEEE round-to-nearest, no fast-math; the
+ * All arithmetic is fp32.  Sums, products and differences are IEEE round-to-nearest; the
+ * scale factor sqrt(c_S / sum) is evaluated as sqrtf(c_S) * rsqrt.approx.ftz(sum) (MUFU.RSQ, <= 2 ulp; build with
+ * -DSMRE_PRECISE_SCALE for sqrt_rn(div_rn())), which is why thresholds must be normal floats (>= FLT_MIN).  The
  * comparison is strict (project iff sum > c_S, Eq. 14).  Images are dense row-major
  * [batch][H][W] fp32, idx = (b*H + row)*W + col, frames independent.
  *
@@ -99,6 +101,29 @@ smre_status smre_project(smre_handle h, const float *y_dev, float *x_out_dev,
  */
 smre_status smre_project_host(smre_handle h, const float *y_host, float *x_out_host,
                               int n_sweeps, void *cuda_stream);
+
+/*
+ * Projection under the paper's own stopping rules instead of a fixed count (the paper "runs Dykstra until
+ * convergence", tol 1e-3: PAPER.md:571, 752).  The decision is taken on the device; nothing returns to the host.
+ *   SMRE_STANDARD   Alg. 2: stop after the first sweep r with ||x_r - x_{r-1}||_2^2 <= tol (tol is
+ *                   Alg. 2's delta; x_0 = y), at most max_sweeps sweeps, each frame on its own.  The squared norm is
+ *                   accumulated in fp32 per thread and in fp64 above (fixed order: the same input stops on the same
+ *                   sweep every time).  Runs on the strip scheduler; SMRE_EUNSUPPORTED where that does not take the
+ *                   problem.  sweeps_done_dev: DEVICE int[batch] or NULL, receives r per frame.
+ *   SMRE_INCOMPLETE Listing 3: within each shift every L x L tile (L = 2^K) iterates until the
+ *                   sum over its pixels and the cycle's levels of |x_old - x_new| is <= tol * L^2 (fp32), at most
+ *                   max_sweeps cycles.  sweeps_done_dev: DEVICE int[1] or NULL, receives the largest cycle count of
+ *                   any tile; smre_export_tile_cycles gives all of them.
+ * tol >= 0.  Everything else as smre_project.
+ */
+smre_status smre_project_tol(smre_handle h, const float *y_dev, float *x_out_dev, int max_sweeps, float tol,
+                             int *sweeps_done_dev, void *cuda_stream);
+
+/* SMRE_INCOMPLETE: the cycles every tile ran in shift `shift` (0..K) of the last smre_project_tol, copied to
+ * cycles_out_dev (DEVICE, [batch][tiles_y][tiles_x] ints, may be NULL to query the sizes only).  Tiles of a shift start
+ * at (2^shift mod L) - L on both axes, those entirely above / left of the image left out. */
+smre_status smre_export_tile_cycles(smre_handle h, int shift, int *cycles_out_dev, int *tiles_y, int *tiles_x,
+                                    void *cuda_stream);
 
 /* Frees every device and host resource of the handle.  NULL is accepted. */
 smre_status smre_destroy(smre_handle h);

@@ -59,6 +59,8 @@ struct smre_handle_s {
     // incomplete
     int K = 0;
     IcdLevels levels{};
+    int *tile_cycles = nullptr;        // cycles every tile ran in the last smre_project_tol, shift-major
+    std::vector<size_t> tile_off;      // offset of shift i in tile_cycles; [K + 1] = total
     // host staging for smre_project_host
     float *stage_in = nullptr, *stage_out = nullptr;
     // last launch
@@ -163,6 +165,15 @@ extern "C" smre_status smre_create(smre_handle *out, int H, int W, int batch, co
             h->levels.c[k] = c_table[a];
             h->levels.sqrt_c[k] = sqrtf(c_table[a]);
         }
+        h->tile_off.assign(K + 2, 0);
+        for (int i = 0; i <= K; ++i)
+            h->tile_off[i + 1] = h->tile_off[i] + (size_t)batch * icd_tiles_along(H, K, i) * icd_tiles_along(W, K, i);
+        if (cudaMalloc(&h->tile_cycles, h->tile_off[K + 1] * sizeof(int)) != cudaSuccess ||
+            cudaMemset(h->tile_cycles, 0, h->tile_off[K + 1] * sizeof(int)) != cudaSuccess) {
+            cudaGetLastError();
+            smre_destroy(h);
+            return fail(SMRE_ENOMEM, "allocating the per-tile cycle counters failed");
+        }
         for (int i = 0; i <= K; ++i)
             for (int k = K; k >= i; --k) {
                 const int side = 1 << k, o = (1 << i) % side;
@@ -184,6 +195,7 @@ extern "C" smre_status smre_destroy(smre_handle h)
     if (h->sweep_graph) cudaGraphExecDestroy(h->sweep_graph);
     if (h->q) cudaFree(h->q);
     if (h->xwork) cudaFree(h->xwork);
+    if (h->tile_cycles) cudaFree(h->tile_cycles);
     if (h->stage_in) cudaFree(h->stage_in);
     if (h->stage_out) cudaFree(h->stage_out);
     delete h;
@@ -258,6 +270,74 @@ extern "C" smre_status smre_project(smre_handle h, const float *y_dev, float *x_
     for (int s = 0; s < n_sweeps; ++s) CU(cudaGraphLaunch(h->sweep_graph, st));
     CU(cudaMemcpyAsync(x_out_dev, h->xwork, bytes, cudaMemcpyDeviceToDevice, st));
     h->last_launches = (long long)n_sweeps * (long long)h->fams.size();
+    return SMRE_OK;
+}
+
+// max over ints (the largest cycle count of any tile), one block
+__global__ void max_int_kernel(const int *v, size_t n, int *out)
+{
+    __shared__ int sm[32];
+    int m = 0;
+    for (size_t i = threadIdx.x; i < n; i += blockDim.x) m = max(m, v[i]);
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < (int)(blockDim.x >> 5); ++k) m = max(m, sm[k]);
+        *out = m;
+    }
+}
+
+extern "C" smre_status smre_project_tol(smre_handle h, const float *y_dev, float *x_out_dev, int max_sweeps, float tol,
+                                        int *sweeps_done_dev, void *cuda_stream)
+{
+    if (!h) return fail(SMRE_EINVAL, "handle is NULL");
+    if (!y_dev || !x_out_dev) return fail(SMRE_EINVAL, "y_dev / x_out_dev is NULL");
+    if (max_sweeps <= 0) return fail(SMRE_EINVAL, "max_sweeps must be positive");
+    if (!(tol >= 0.0f) || !std::isfinite(tol)) return fail(SMRE_EINVAL, "tol must be finite and >= 0");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    h->last_launches = 0;
+    if (h->variant == SMRE_INCOMPLETE) {
+        // Listing 2 + the while loop of Listing 3: per shift, every tile until its own stop
+        h->last_schedule = SMRE_SCHED_GRAPH;
+        for (int i = 0; i <= h->K; ++i) {
+            const float *src = (i == 0) ? y_dev : x_out_dev;
+            CU(launch_icd_shift_tol(src, x_out_dev, h->B, h->H, h->W, h->K, i, h->levels, max_sweeps, st, true, tol,
+                                    h->tile_cycles + h->tile_off[i]));
+            ++h->last_launches;
+        }
+        if (sweeps_done_dev) {
+            max_int_kernel<<<1, 256, 0, st>>>(h->tile_cycles, h->tile_off[h->K + 1], sweeps_done_dev);
+            CU(cudaGetLastError());
+            ++h->last_launches;
+        }
+        return SMRE_OK;
+    }
+    if (!h->strips)
+        return fail(SMRE_EUNSUPPORTED, "convergence control of the standard variant runs on the strip scheduler, which "
+                                       "does not take this problem: %s", h->strips_why);
+    if (h->last_schedule == SMRE_SCHED_STRIPS && strips_plan_status(h->strips) != 0)
+        return fail(SMRE_ECUDA, "the previous projection on this handle failed: a wait of the strip scheduler timed out "
+                                "(code 0x%x), its result is invalid", strips_plan_status(h->strips));
+    cudaError_t e = strips_run_tol(h->strips, y_dev, x_out_dev, max_sweeps, true, tol, sweeps_done_dev, st, &h->last_launches);
+    if (e == cudaErrorNotSupported) return fail(SMRE_EUNSUPPORTED, "the strip scheduler has no room for x_{r-1} at this width");
+    if (e != cudaSuccess) return cuda_fail(e, "strips_run_tol");
+    h->last_schedule = SMRE_SCHED_STRIPS;
+    return SMRE_OK;
+}
+
+extern "C" smre_status smre_export_tile_cycles(smre_handle h, int shift, int *cycles_out_dev, int *tiles_y, int *tiles_x,
+                                               void *cuda_stream)
+{
+    if (!h) return fail(SMRE_EINVAL, "handle is NULL");
+    if (h->variant != SMRE_INCOMPLETE) return fail(SMRE_EUNSUPPORTED, "only the incomplete variant iterates tile by tile");
+    if (shift < 0 || shift > h->K) return fail(SMRE_EINVAL, "shift %d outside [0, %d]", shift, h->K);
+    if (tiles_y) *tiles_y = icd_tiles_along(h->H, h->K, shift);
+    if (tiles_x) *tiles_x = icd_tiles_along(h->W, h->K, shift);
+    if (cycles_out_dev)
+        CU(cudaMemcpyAsync(cycles_out_dev, h->tile_cycles + h->tile_off[shift],
+                           (h->tile_off[shift + 1] - h->tile_off[shift]) * sizeof(int), cudaMemcpyDeviceToDevice,
+                           (cudaStream_t)cuda_stream));
     return SMRE_OK;
 }
 

@@ -59,4 +59,11 @@ struct IcdLevels {
 cudaError_t launch_icd_shift(const float *src, float *dst, int B, int H, int W, int K, int shift_i,
                              const IcdLevels &lv, int n_cycles, cudaStream_t st);
 
+// Same with the stop rule of Listing 3: every tile iterates until its sum |x_old - x_new| of one
+// cycle is <= tol * L^2, at most n_cycles cycles.  tile_cycles: null or [B][tiles_y][tiles_x] ints (icd_tiles_along).
+cudaError_t launch_icd_shift_tol(const float *src, float *dst, int B, int H, int W, int K, int shift_i,
+                                 const IcdLevels &lv, int n_cycles, cudaStream_t st, bool use_tol, float tol,
+                                 int *tile_cycles);
+int icd_tiles_along(int N, int K, int shift_i);
+
 }  // namespace smre

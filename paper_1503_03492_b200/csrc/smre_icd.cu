@@ -24,10 +24,15 @@ __device__ __forceinline__ int morton_even_bits(int t) {   // bits 0,2,4 of t ->
 // 2x2 gives four times the lanes and a shorter dependent chain per level pass, which wins when the whole
 // problem is too small to fill the machine (C2: 512^2, K = 3).  Tiles of 16x16 and 32x32 need 4x4 (a tile
 // must fit in two warps).
-template <int K, int LP>
+// TOL: the stop rule of Listing 3: a tile stops after the first cycle whose sum over the
+// tile's pixels and the cycle's levels of |x_old - x_new| is <= thresh = tol * L^2 (fp32; the lanes of a tile add
+// their parts with an xor-shuffle tree), or after n_cycles cycles.  Tiles that have stopped keep x and q frozen
+// while other tiles of the warp go on.  tile_cycles (may be null): cycles every tile ran.
+template <int K, int LP, bool TOL>
 __global__ void __launch_bounds__(128)
 icd_shift_kernel(const float *src, float *dst, int H, int W, int org,
-                 int nty, int ntx, long long n_tiles, int smin, IcdLevels lv, int n_cycles)
+                 int nty, int ntx, long long n_tiles, int smin, IcdLevels lv, int n_cycles,
+                 float thresh, int *tile_cycles)
 {
     constexpr int L = 1 << K;
     constexpr int P = 1 << LP;                    // pixel block edge per lane: 1, 2, 2, 2, 4, 4
@@ -98,8 +103,16 @@ icd_shift_kernel(const float *src, float *dst, int H, int W, int org,
         for (int p = 0; p < NP; ++p) q[k][p] = 0.0f;              // "Set q = 0"
 
     __shared__ float red[4];
+    __shared__ float dred[4];
+    bool active = true;                                           // TOL: the lane's tile still iterates
+    int my_cycles = 0;
 
     for (int cyc = 0; cyc < n_cycles; ++cyc) {
+        float delta = 0.0f;                                       // TOL: sum |x_old - x_new| of my pixels, this cycle
+        if (TOL) {
+            if (LPT > 32) { if (!__syncthreads_or(active)) break; }          // a tile spans two warps
+            else if (!__any_sync(0xffffffffu, active)) break;
+        }
         // coarse -> fine: for (s = K; s >= smin; s--)
 #pragma unroll
         for (int k = K; k >= 0; --k) {
@@ -129,8 +142,11 @@ icd_shift_kernel(const float *src, float *dst, int H, int W, int org,
 #pragma unroll
                 for (int p = 0; p < NP; ++p) {
                     const float xn = alpha * v[p];
-                    q[k][p] = v[p] - xn;
-                    x[p] = xn;
+                    if (!TOL || active) {
+                        if (TOL) delta += fabsf(x[p] - xn);
+                        q[k][p] = v[p] - xn;
+                        x[p] = xn;
+                    }
                 }
             } else {
                 // ---- windows inside the lane's block ------------------------------------------
@@ -157,13 +173,32 @@ icd_shift_kernel(const float *src, float *dst, int H, int W, int org,
                             for (int c = 0; c < S; ++c) {
                                 const int p = (wy * S + r) * P + wx * S + c;
                                 const float xn = alpha * v[r * S + c];
-                                q[k][p] = v[r * S + c] - xn;
-                                x[p] = xn;
+                                if (!TOL || active) {
+                                    if (TOL) delta += fabsf(x[p] - xn);
+                                    q[k][p] = v[r * S + c] - xn;
+                                    x[p] = xn;
+                                }
                             }
                     }
             }
         }
+        if (TOL) {                                                // the tile's delta: tree over its LPT lanes
+#pragma unroll
+            for (int m = 1; m < 32; m <<= 1)
+                if (m < LPT) delta += __shfl_xor_sync(0xffffffffu, delta, m);
+            if (LPT > 32) {
+                const int w = threadIdx.x >> 5;
+                if ((threadIdx.x & 31) == 0) dred[w] = delta;
+                __syncthreads();
+                delta = dred[w & ~1] + dred[w | 1];
+            }
+            if (active) {
+                ++my_cycles;
+                if (!(delta > thresh)) active = false;            // while (delta > tol*1024)
+            }
+        }
     }
+    if (TOL && tile_cycles && tile_ok && t == 0) tile_cycles[tile] = my_cycles;
 
 #pragma unroll
     for (int r = 0; r < P; ++r)
@@ -175,7 +210,8 @@ icd_shift_kernel(const float *src, float *dst, int H, int W, int org,
 
 template <int K, int LP>
 static cudaError_t launch_kp(const float *src, float *dst, int B, int H, int W, int shift_i,
-                             const IcdLevels &lv, int n_cycles, cudaStream_t st)
+                             const IcdLevels &lv, int n_cycles, cudaStream_t st, bool use_tol, float tol,
+                             int *tile_cycles)
 {
     constexpr int L = 1 << K;
     constexpr int P = 1 << LP;
@@ -187,34 +223,53 @@ static cudaError_t launch_kp(const float *src, float *dst, int B, int H, int W, 
     const long long lanes = n_tiles * LPT;
     const int threads = 128;
     const long long blocks = (lanes + threads - 1) / threads;
-    icd_shift_kernel<K, LP><<<(unsigned)blocks, threads, 0, st>>>(src, dst, H, W, org, nty, ntx, n_tiles,
-                                                             shift_i, lv, n_cycles);
+    if (use_tol)
+        icd_shift_kernel<K, LP, true><<<(unsigned)blocks, threads, 0, st>>>(src, dst, H, W, org, nty, ntx, n_tiles, shift_i, lv,
+                                                                       n_cycles, tol * (float)(L * L), tile_cycles);
+    else
+        icd_shift_kernel<K, LP, false><<<(unsigned)blocks, threads, 0, st>>>(src, dst, H, W, org, nty, ntx, n_tiles, shift_i, lv,
+                                                                        n_cycles, 0.0f, nullptr);
     return cudaGetLastError();
 }
 
 template <int K>
 static cudaError_t launch_k(const float *src, float *dst, int B, int H, int W, int shift_i,
-                            const IcdLevels &lv, int n_cycles, cudaStream_t st)
+                            const IcdLevels &lv, int n_cycles, cudaStream_t st, bool use_tol, float tol,
+                            int *tile_cycles)
 {
     constexpr int LPmax = K < 2 ? K : 2;                   // 4x4 blocks where the tile allows it
     if constexpr (K == 2 || K == 3) {
         // lanes the 4x4 layout would give; below about half a machine of resident threads use 2x2 blocks
         const long long lanes4 = (long long)B * ((H + (1 << K) - 1) >> K) * ((W + (1 << K) - 1) >> K) * (1 << (2 * (K - 2)));
-        if (lanes4 < 148ll * 1024) return launch_kp<K, 1>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
+        if (lanes4 < 148ll * 1024) return launch_kp<K, 1>(src, dst, B, H, W, shift_i, lv, n_cycles, st, use_tol, tol, tile_cycles);
     }
-    return launch_kp<K, LPmax>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
+    return launch_kp<K, LPmax>(src, dst, B, H, W, shift_i, lv, n_cycles, st, use_tol, tol, tile_cycles);
+}
+
+// tiles of shift i along an axis of extent N (tile edge 2^K): the layout of the per-tile cycle counts
+int icd_tiles_along(int N, int K, int shift_i)
+{
+    const int L = 1 << K, o = (1 << shift_i) % L, org = o ? o - L : 0;
+    return (N - org + L - 1) / L;
 }
 
 cudaError_t launch_icd_shift(const float *src, float *dst, int B, int H, int W, int K, int shift_i,
                              const IcdLevels &lv, int n_cycles, cudaStream_t st)
 {
+    return launch_icd_shift_tol(src, dst, B, H, W, K, shift_i, lv, n_cycles, st, false, 0.0f, nullptr);
+}
+
+cudaError_t launch_icd_shift_tol(const float *src, float *dst, int B, int H, int W, int K, int shift_i,
+                                 const IcdLevels &lv, int n_cycles, cudaStream_t st, bool use_tol, float tol,
+                                 int *tile_cycles)
+{
     switch (K) {
-        case 0: return launch_k<0>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
-        case 1: return launch_k<1>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
-        case 2: return launch_k<2>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
-        case 3: return launch_k<3>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
-        case 4: return launch_k<4>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
-        case 5: return launch_k<5>(src, dst, B, H, W, shift_i, lv, n_cycles, st);
+        case 0: return launch_k<0>(src, dst, B, H, W, shift_i, lv, n_cycles, st, use_tol, tol, tile_cycles);
+        case 1: return launch_k<1>(src, dst, B, H, W, shift_i, lv, n_cycles, st, use_tol, tol, tile_cycles);
+        case 2: return launch_k<2>(src, dst, B, H, W, shift_i, lv, n_cycles, st, use_tol, tol, tile_cycles);
+        case 3: return launch_k<3>(src, dst, B, H, W, shift_i, lv, n_cycles, st, use_tol, tol, tile_cycles);
+        case 4: return launch_k<4>(src, dst, B, H, W, shift_i, lv, n_cycles, st, use_tol, tol, tile_cycles);
+        case 5: return launch_k<5>(src, dst, B, H, W, shift_i, lv, n_cycles, st, use_tol, tol, tile_cycles);
         default: return cudaErrorInvalidValue;
     }
 }

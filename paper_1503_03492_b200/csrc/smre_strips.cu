@@ -41,6 +41,13 @@ struct StripArgs {
     int side[ST_MAX_SIDES], fam_base[ST_MAX_SIDES];
     float c[ST_MAX_SIDES], sqrt_c[ST_MAX_SIDES];
     unsigned tag_base;
+    // convergence control (Alg. 2: "while ||x_r - x_{r-1}||^2 > delta"); tol_mode 0: fixed n_sweeps
+    int tol_mode;
+    float delta;
+    int NR_total;                   // ring rows the shared-memory layout was made for (NR of them are used as ring)
+    double *partials;               // [2][cta]: this CTA's part of ||x_r - x_{r-1}||^2, by sweep parity
+    unsigned *sweep_ctr;            // [frame of the launch][32]: CTAs that have delivered their part (monotonic)
+    int *sweeps_done;               // [Btot] or null: sweeps run per frame
     int elim;                       // 1: stores that would not change memory are not issued
     unsigned long long timeout_ns;
 #ifdef SMRE_ST_KO
@@ -124,7 +131,7 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 // A wait that does not come true within A.timeout_ns raises the device status word and the CTA's abort flag; from
 // then on every wait of the CTA returns at once (and other CTAs see the status word in their slow path), so a
 // protocol bug or a lost CTA ends the kernel with an error code instead of hanging the GPU.
-enum { ST_W_QFULL = 1, ST_W_MAIL = 4, ST_W_DONE = 6 };
+enum { ST_W_QFULL = 1, ST_W_ALLOW = 3, ST_W_MAIL = 4, ST_W_SWEEP = 5, ST_W_DONE = 6 };
 
 struct Waiter {
     const StripArgs &A;
@@ -481,9 +488,10 @@ __device__ __forceinline__ void macro_step(const StripArgs &A, const MacroEntry 
 //     one-sweep dependency (the rows of step h were written in step h - F) allow.  It reads `progress` with acquire
 //     semantics and orders its async-proxy reads behind the generic-proxy writes with a proxy fence.
 __device__ void waiter_warp(const StripArgs &A, const MacroEntry *tab, int M, uint64_t *full, unsigned *progress,
-                            unsigned *abort_flag, int lane, int NTL)
+                            unsigned *abort_flag, const unsigned *stopped, int lane, int NTL)
 {
     Waiter wt(A, abort_flag);
+    const bool tol_mode = A.tol_mode != 0;
     const bool off = ST_KO(A, 2);
     const int total = A.n_sweeps * A.F;
     unsigned cn = 0;                           // staged non-empty steps consumed
@@ -491,7 +499,22 @@ __device__ void waiter_warp(const StripArgs &A, const MacroEntry *tab, int M, ui
 #ifdef SMRE_ST_KO
     long long t_wait = 0, t_bar = 0; int n_late = 0;
 #endif
-    for (int sweep = 0; sweep < A.n_sweeps; ++sweep)
+    for (int sweep = 0; sweep < A.n_sweeps; ++sweep) {
+        if (tol_mode && sweep > 0) {
+            // top of a sweep under convergence control: the compute warps decide (barrier A); if the run goes on, the
+            // q rows of the sweep's first family are awaited here, since nothing was issued across the decision
+            bar_sync(3, NTL);
+            if (*(volatile const unsigned *)stopped) return;
+            if (!off && tab[0].rows > 0) {
+                const unsigned stage = cn % ST_NSTG, parity = (cn / ST_NSTG) & 1u;
+                if (!mbar_try_wait(&full[stage], parity)) {
+                    wt.begin();
+                    while (!mbar_try_wait(&full[stage], parity))
+                        if (wt.slow(ST_W_QFULL)) break;
+                }
+            }
+            bar_sync(3, NTL);
+        }
         for (int m = 0; m < M; ++m) {
             const int crows = tab[m].rows, cs_ = tab[m].s;
             const int nrows_macro = tab[(m + 1 == M) ? 0 : m + 1].rows;
@@ -499,7 +522,8 @@ __device__ void waiter_warp(const StripArgs &A, const MacroEntry *tab, int M, ui
             for (int ox = 0; ox < cs_; ++ox, ++g) {
                 const bool last_ox = ox + 1 == cs_;
                 const int nrows = last_ox ? nrows_macro : crows;
-                const bool nstaged = (last_ox && m + 1 == M) ? true : sweep > 0;
+                const bool sweep_end = last_ox && m + 1 == M;
+                const bool nstaged = sweep_end ? !tol_mode : sweep > 0;       // tol mode: see the top of the sweep
                 if (!off && g + 1 < total && nstaged && nrows > 0) {
                     const unsigned n1 = cn + (cur_staged ? 1u : 0u);
                     const unsigned stage = n1 % ST_NSTG, parity = (n1 / ST_NSTG) & 1u;
@@ -529,6 +553,7 @@ __device__ void waiter_warp(const StripArgs &A, const MacroEntry *tab, int M, ui
 #endif
             }
         }
+    }
 #ifdef SMRE_ST_KO
     if ((A.ko & 256) && lane == 0 && (blockIdx.x % 40) == 3)
         printf("waiter cta %d: steps %d  q-wait %lld cycles/step  late %d  barrier+release %lld cycles/step\n", blockIdx.x, g,
@@ -555,7 +580,8 @@ __device__ __forceinline__ void staged_skip_empty(StagedCursor &k, const MacroEn
 
 template <int PITCH>
 __device__ void issuer_warp(const StripArgs &A, const MacroEntry *tab, int M, float *ring, uint64_t *full,
-                            unsigned *progress, unsigned *abort_flag, int frame, int lane)
+                            unsigned *progress, unsigned *abort_flag, const unsigned *allow, const unsigned *stopped,
+                            int frame, int lane)
 {
     constexpr int KMAX = 4;                                     // steps per batch (bookkeeping stays in registers)
     const int pitch = PITCH ? PITCH : A.Wq;
@@ -610,6 +636,18 @@ __device__ void issuer_warp(const StripArgs &A, const MacroEntry *tab, int M, fl
             if (++tail.ox == tab[tail.m].s) { tail.ox = 0; if (++tail.m == M) tail.m = 0; }
             staged_skip_empty(tail, tab, M, total);
         }
+        if (A.tol_mode) {
+            // under convergence control nothing of a sweep is loaded before the sweep has been decided: a copy in
+            // flight into the shared memory of a CTA that has stopped would outlive it
+            const unsigned sweep_of_batch = (unsigned)(head.g / F);
+            if (ld_acquire_cta(allow) <= sweep_of_batch) {
+                wt.begin();
+                while (ld_acquire_cta(allow) <= sweep_of_batch) {
+                    if (*(volatile const unsigned *)stopped) return;
+                    if (wt.slow(ST_W_ALLOW)) break;
+                }
+            }
+        }
         if (have < need) {
             wt.begin();
             while ((have = ld_acquire_cta(progress)) < need)
@@ -649,10 +687,14 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
     const int T = A.T, TR = st_tile_rows(T);
     float *tile = reinterpret_cast<float *>(smem_raw);
     float *ring = tile + TR * pitch;
-    uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)A.NR * pitch);
+    float *xprev = ring + (size_t)A.NR * pitch;                 // tol mode: x_{r-1} of the rows held at the top of a sweep
+    uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)A.NR_total * pitch);
     MacroEntry *tab = reinterpret_cast<MacroEntry *>(full + ST_NSTG);
     unsigned *abort_flag = reinterpret_cast<unsigned *>(tab + ST_MAX_SIDES * ST_MAX_SIDE);
     unsigned *progress = abort_flag + 1;
+    unsigned *allow = abort_flag + 2;                           // tol mode: sweeps the run is allowed to execute so far
+    unsigned *stopped = abort_flag + 3;                         // tol mode: the stop rule has fired
+    double *wsum = reinterpret_cast<double *>(abort_flag + 4);  // [ST_MAX_WARPS + 1] per-warp parts of ||x_r - x_{r-1}||^2
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int NWC = A.NWC, NT = NWC * 32, NTL = NT + (ST_KO(A, 32) ? 0 : 32);
@@ -705,14 +747,16 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
         for (int i = 0; i < ST_NSTG; ++i) mbar_init(&full[i], 1);
         *abort_flag = 0u;
         *progress = 0u;
+        *allow = A.tol_mode ? 1u : (unsigned)A.n_sweeps;
+        *stopped = 0u;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
     if (warp == NWC) {
-        if (!ST_KO(A, 32)) waiter_warp(A, tab, M, full, progress, abort_flag, lane, NTL);
+        if (!ST_KO(A, 32)) waiter_warp(A, tab, M, full, progress, abort_flag, stopped, lane, NTL);
     } else if (warp == NWC + 1) {
-        issuer_warp<PITCH>(A, tab, M, ring, full, progress, abort_flag, frame, lane);
+        issuer_warp<PITCH>(A, tab, M, ring, full, progress, abort_flag, allow, stopped, frame, lane);
     } else {
         const int tid = threadIdx.x;
         const int slot_base = T / 2 - j * T;
@@ -728,7 +772,55 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
 #endif
         cs.seen_m3 = cs.seen_m2 = cs.seen_m1 = cs.seen_p1 = cs.seen_p2 = cs.seen_p3 = A.tag_base;
         Waiter wt(A, abort_flag);
-        for (int sweep = 0; sweep < A.n_sweeps; ++sweep)
+        bool stopped_early = false;
+        const int h_lo = tab[0].hold_lo, h_hi = tab[0].hold_hi;      // rows held at the top of EVERY sweep
+        for (int sweep = 0; sweep < A.n_sweeps; ++sweep) {
+            if (A.tol_mode) {
+                // ---- Alg. 2's stop rule: after sweep r, stop if ||x_r - x_{r-1}||^2 <= delta ----------
+                if (sweep > 0) {
+                    float acc = 0.0f;                            // my columns of the rows I hold (same rows as a sweep ago)
+                    for (int y = h_lo; y < h_hi; ++y)
+                        for (int c = tid; c < W; c += NT) {
+                            const float d = tile[(y + slot_base) * pitch + c] - xprev[(y - h_lo) * pitch + c];
+                            acc = fmaf(d, d, acc);
+                        }
+                    double part = (double)acc;                   // fixed order from here on: deterministic decision
+#pragma unroll
+                    for (int m2 = 1; m2 < 32; m2 <<= 1) part += __shfl_xor_sync(0xffffffffu, part, m2);
+                    if (lane == 0) wsum[warp] = part;
+                    bar_sync(2, NT);
+                    if (tid == 0) {
+                        double mine = 0.0;
+                        for (int k = 0; k < NWC; ++k) mine += wsum[k];
+                        A.partials[(size_t)(sweep & 1) * gridDim.x + cta] = mine;
+                        __threadfence();
+                        atomicAdd(A.sweep_ctr + (size_t)fl * 32, 1u);
+                        // every strip of the frame has delivered its part of this sweep
+                        const unsigned need = (unsigned)NS * (unsigned)sweep;
+                        unsigned got;
+                        wt.begin();
+                        for (;;) {
+                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(got) : "l"(A.sweep_ctr + (size_t)fl * 32) : "memory");
+                            if (got >= need || wt.slow(ST_W_SWEEP)) break;
+                        }
+                        double d2 = 0.0;
+                        const double *pp = A.partials + (size_t)(sweep & 1) * gridDim.x + (size_t)fl * NS;
+                        for (int k = 0; k < NS; ++k) d2 += __ldcg(pp + k);
+                        const bool stop = !(d2 > (double)A.delta);
+                        if (stop) {
+                            *(volatile unsigned *)stopped = 1u;
+                            if (j == 0 && A.sweeps_done) A.sweeps_done[frame] = sweep;
+                        } else {
+                            st_release_cta(allow, (unsigned)sweep + 1u);      // the issuer may load this sweep's rows
+                        }
+                    }
+                    bar_sync(3, NTL);                            // A: decision published (compute warps + waiter)
+                    if (*(volatile unsigned *)stopped) { stopped_early = true; break; }
+                }
+                for (int y = h_lo; y < h_hi; ++y)                // x_{r-1} for the next check
+                    for (int c = tid; c < W; c += NT) xprev[(y - h_lo) * pitch + c] = tile[(y + slot_base) * pitch + c];
+                if (sweep > 0) bar_sync(3, NTL);                 // B: the waiter has the first family's q rows
+            }
             for (int m = 0; m < M; ++m) {
                 const MacroEntry e = tab[m];
                 const bool staged = sweep > 0 && !ST_KO(A, 2);
@@ -742,14 +834,18 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
                 if (!handoff) break;
                 transition(A, tile, pitch, j, cta, e, cs, tid, NT, wt);
             }
+        }
+        if (A.tol_mode && !stopped_early && j == 0 && tid == 0 && A.sweeps_done) A.sweeps_done[frame] = A.n_sweeps;
 #ifdef SMRE_ST_KO
         if ((A.ko & 256) && (tid == 0 || tid == 200) && (j == NS / 2 || j == NS / 2 + 1 || j == 3))
             printf("strip %d tid %d: transitions %u  send %lld  recv %lld  bar %lld  macro %lld cycles (avg per transition)\n", j, tid,
                    cs.mc, cs.t_send / max(cs.mc, 1u), cs.t_recv / max(cs.mc, 1u), cs.t_bar / max(cs.mc, 1u), cs.t_macro / max(cs.mc, 1u));
 #endif
         // row a9: the rows the strip holds under the last family's geometry
+        // (after an early stop: under the first family's, which a strip holds at the top of every sweep)
         float *xo = A.x_out + (size_t)frame * H * W;
-        for (int y = tab[M - 1].hold_lo; y < tab[M - 1].hold_hi; ++y)
+        const int o_lo = stopped_early ? h_lo : tab[M - 1].hold_lo, o_hi = stopped_early ? h_hi : tab[M - 1].hold_hi;
+        for (int y = o_lo; y < o_hi; ++y)
             for (int c = tid; c < W; c += NT) xo[(size_t)y * W + c] = tile[(y + slot_base) * pitch + c];
     }
     __syncthreads();
@@ -771,7 +867,8 @@ struct StripPlan {
     float c[ST_MAX_SIDES] = {}, sqrt_c[ST_MAX_SIDES] = {};
     float *q = nullptr;
     unsigned long long *mail = nullptr;
-    unsigned *done = nullptr, *status = nullptr, *finished = nullptr;
+    unsigned *done = nullptr, *status = nullptr, *finished = nullptr, *sweep_ctr = nullptr;
+    double *partials = nullptr;
     unsigned *status_host = nullptr;                             // pinned, mapped
     unsigned *status_host_dev = nullptr;
     size_t mail_bytes = 0, smem_bytes = 0;
@@ -792,7 +889,7 @@ static void set_why(char *why, size_t n, const char *fmt, ...)
     va_end(ap);
 }
 
-static size_t strips_fixed_smem() { return ST_NSTG * 8 + ST_MAX_SIDES * ST_MAX_SIDE * sizeof(MacroEntry) + 16; }
+static size_t strips_fixed_smem() { return ST_NSTG * 8 + ST_MAX_SIDES * ST_MAX_SIDE * sizeof(MacroEntry) + 16 + (ST_MAX_WARPS + 2) * 8; }
 
 // Brute-force check of one strip height against every geometry of a sweep (host only, closed forms).
 static bool strips_check_T(int H, int NS, int T, const int *sides, int n_sides, int *max_rows, int *max_hop,
@@ -927,6 +1024,8 @@ StripPlan *strips_plan_create(int H, int W, int B, int Wq, const int *sides, con
     if (e == cudaSuccess) e = cudaMalloc(&p->mail, p->mail_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&p->done, ctas * 128);
     if (e == cudaSuccess) e = cudaMalloc(&p->status, 256);
+    if (e == cudaSuccess) e = cudaMalloc(&p->partials, 2 * ctas * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&p->sweep_ctr, (size_t)p->frames_per_launch * 128);
     if (e == cudaSuccess) e = cudaHostAlloc(&p->status_host, 64, cudaHostAllocMapped);
     if (e == cudaSuccess) e = cudaHostGetDevicePointer(&p->status_host_dev, p->status_host, 0);
     if (e == cudaSuccess) e = cudaMemset(p->mail, 0, p->mail_bytes);
@@ -952,6 +1051,8 @@ void strips_plan_destroy(StripPlan *p)
     if (p->mail) cudaFree(p->mail);
     if (p->done) cudaFree(p->done);
     if (p->status) cudaFree(p->status);
+    if (p->partials) cudaFree(p->partials);
+    if (p->sweep_ctr) cudaFree(p->sweep_ctr);
     if (p->status_host) cudaFreeHost(p->status_host);
     delete p;
 }
@@ -966,6 +1067,14 @@ int strips_plan_status(const StripPlan *p) { return (int)*(volatile unsigned *)p
 
 cudaError_t strips_run(StripPlan *p, const float *y, float *x_out, int n_sweeps, cudaStream_t st, long long *launches)
 {
+    return strips_run_tol(p, y, x_out, n_sweeps, false, 0.0f, nullptr, st, launches);
+}
+
+cudaError_t strips_run_tol(StripPlan *p, const float *y, float *x_out, int n_sweeps, bool tol_mode, float delta,
+                           int *sweeps_done, cudaStream_t st, long long *launches)
+{
+    const int xprev_rows = tol_mode ? st_tile_rows(p->T) : 0;           // x_{r-1} is taken out of the q ring
+    if (p->NR - xprev_rows < 3 * p->max_rows + 8) return cudaErrorNotSupported;
     int M = 0;
     for (int a = 0; a < p->n_sides; ++a) M += p->side[a];
     const unsigned long long total = (unsigned long long)n_sweeps * M + 2;
@@ -986,7 +1095,13 @@ cudaError_t strips_run(StripPlan *p, const float *y, float *x_out, int n_sweeps,
         A.status = p->status; A.status_host = p->status_host_dev; A.finished = p->finished;
         A.H = p->H; A.W = p->W; A.Wq = p->Wq; A.Btot = p->B; A.frame0 = f0;
         A.T = p->T; A.NS = p->NS; A.NWC = p->NWC; A.n_sides = p->n_sides; A.F = p->F; A.n_sweeps = n_sweeps;
-        A.NR = p->NR; A.max_rows = p->max_rows;
+        A.NR = p->NR - xprev_rows; A.NR_total = p->NR; A.max_rows = p->max_rows;
+        A.tol_mode = tol_mode ? 1 : 0; A.delta = delta; A.partials = p->partials; A.sweep_ctr = p->sweep_ctr;
+        A.sweeps_done = sweeps_done;
+        if (tol_mode) {
+            e = cudaMemsetAsync(p->sweep_ctr, 0, (size_t)p->frames_per_launch * 128, st);
+            if (e != cudaSuccess) return e;
+        }
         for (int a = 0; a < p->n_sides; ++a) {
             A.side[a] = p->side[a]; A.fam_base[a] = p->fam_base[a]; A.c[a] = p->c[a]; A.sqrt_c[a] = p->sqrt_c[a];
         }

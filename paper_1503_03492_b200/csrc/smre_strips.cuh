@@ -68,5 +68,10 @@ void strips_plan_shape(const StripPlan *p, int *strips, int *warps);
 // kernel's epilogue writes: no synchronisation; meaningful once the stream has drained.
 int strips_plan_status(const StripPlan *p);
 cudaError_t strips_run(StripPlan *p, const float *y, float *x_out, int n_sweeps, cudaStream_t st, long long *launches);
+// Same under Alg. 2's stop rule: a frame stops after the first sweep r with ||x_r - x_{r-1}||^2 <= delta,
+// at most n_sweeps sweeps; sweeps_done (device, [B] ints, may be null) receives r per frame.  The decision is taken
+// on the device (one grid barrier per sweep among the strips of a frame); nothing returns to the host.
+cudaError_t strips_run_tol(StripPlan *p, const float *y, float *x_out, int n_sweeps, bool tol_mode, float delta,
+                           int *sweeps_done, cudaStream_t st, long long *launches);
 
 }  // namespace smre

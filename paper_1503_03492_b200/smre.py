@@ -21,7 +21,7 @@ _STATUS = {0: "SMRE_OK", 1: "SMRE_EINVAL", 2: "SMRE_EUNSUPPORTED", 3: "SMRE_ENOM
 exported_symbols = (
     "smre_create", "smre_project", "smre_project_host", "smre_destroy", "smre_set_schedule",
     "smre_info", "smre_family", "smre_export_increments", "smre_last_launch", "smre_last_error",
-    "smre_plan_check", "smre_project_noalloc",
+    "smre_plan_check", "smre_project_noalloc", "smre_project_tol", "smre_export_tile_cycles",
 )
 
 
@@ -62,6 +62,8 @@ def load_library(build_if_missing: bool = True):
     lib.smre_plan_check.argtypes = [ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                     _ip, _ip, _ip, _ip, _llp]
     lib.smre_project_noalloc.argtypes = [ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, _fp, _vp, _vp, ctypes.c_int, _vp]
+    lib.smre_project_tol.argtypes = [_vp, _vp, _vp, ctypes.c_int, ctypes.c_float, _vp, _vp]
+    lib.smre_export_tile_cycles.argtypes = [_vp, ctypes.c_int, _vp, _ip, _ip, _vp]
     for name in exported_symbols:
         getattr(lib, name).restype = ctypes.c_int
     lib.smre_last_error.restype = ctypes.c_char_p
@@ -112,6 +114,18 @@ def smre_project_noalloc(H, W, sides, c_table, y_ptr, x_out_ptr, n_sweeps, strea
         raise ValueError("sides and c_table must be 1-D and of equal length")
     _check(load_library().smre_project_noalloc(int(H), int(W), sides.ctypes.data_as(_ip), len(sides),
                                                c_table.ctypes.data_as(_fp), y_ptr, x_out_ptr, int(n_sweeps), stream))
+
+
+def smre_project_tol(handle, y_ptr, x_out_ptr, max_sweeps, tol, sweeps_done_ptr=None, stream=0):
+    """Projection under the paper's stop rules (Alg. 2 / Listing 3); sweeps_done_ptr: device int address or None."""
+    _check(load_library().smre_project_tol(handle, y_ptr, x_out_ptr, int(max_sweeps), float(tol), sweeps_done_ptr, stream))
+
+
+def smre_export_tile_cycles(handle, shift, out_ptr=None, stream=0):
+    """-> (tiles_y, tiles_x) of the shift; copies the per-tile cycle counts to out_ptr (device ints) if given."""
+    ty, tx = ctypes.c_int(), ctypes.c_int()
+    _check(load_library().smre_export_tile_cycles(handle, int(shift), out_ptr, ctypes.byref(ty), ctypes.byref(tx), stream))
+    return ty.value, tx.value
 
 
 def smre_destroy(handle):
@@ -181,6 +195,33 @@ class Solver:
         st = torch.cuda.current_stream(y.device) if stream is None else stream
         smre_project(self.handle, y.data_ptr(), out.data_ptr(), n_sweeps, st.cuda_stream)
         return out
+
+    def project_tol(self, y, max_sweeps, tol, out=None):
+        """-> (x, sweeps_done int32 tensor: [batch] for the standard variant, [1] = largest tile count for ICD)."""
+        import torch
+        if not (y.is_cuda and y.dtype == torch.float32 and y.is_contiguous()) or y.numel() != self.batch * self.H * self.W:
+            raise ValueError("y must be a contiguous float32 CUDA tensor of batch*H*W elements")
+        if out is None:
+            out = torch.empty_like(y)
+        done = torch.zeros(self.batch if self.variant == SMRE_STANDARD else 1, dtype=torch.int32, device=y.device)
+        st = torch.cuda.current_stream(y.device)
+        smre_project_tol(self.handle, y.data_ptr(), out.data_ptr(), max_sweeps, tol, done.data_ptr(), st.cuda_stream)
+        return out, done
+
+    def tile_cycles(self):
+        """ICD: list per shift of int32 tensors [batch, tiles_y, tiles_x] of the last project_tol."""
+        import torch
+        res, i = [], 0
+        while True:
+            try:
+                ty, tx = smre_export_tile_cycles(self.handle, i)
+            except SmreError:
+                break
+            t = torch.zeros((self.batch, ty, tx), dtype=torch.int32, device="cuda")
+            smre_export_tile_cycles(self.handle, i, t.data_ptr(), torch.cuda.current_stream().cuda_stream)
+            res.append(t)
+            i += 1
+        return res
 
     def project_host(self, y_np, n_sweeps, out=None, stream=0):
         y_np = np.ascontiguousarray(y_np, dtype=np.float32)
