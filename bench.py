@@ -39,6 +39,35 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
 
 
+def profile_metric(workload_name, key):
+    """A per-launch number taken from the committed ncu summaries (profiles/r02_measured.json, written from the
+    captures named there): DRAM traffic of the C1 kernel, thread-instructions of the ICD kernels.  None if absent."""
+    p = os.path.join(ROOT, "profiles", "r02_measured.json")
+    try:
+        d = json.load(open(p))
+        return d.get(workload_name, {}).get(key), "profiles/r02_measured.json (" + d.get("_source", "?") + ")"
+    except (OSError, ValueError):
+        return None, None
+
+
+def cpu_info():
+    """Host description printed beside the oracle timing."""
+    model = "?"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    try:
+        gcc = subprocess.run(["gcc", "--version"], capture_output=True, text=True).stdout.splitlines()[0]
+    except (OSError, IndexError):
+        gcc = "?"
+    from oracle import smre_oracle
+    return {"cpu_model": model, "nproc": os.cpu_count(), "compiler": gcc, "cflags": " ".join(smre_oracle.CFLAGS)}
+
+
 def workload_numbers(w):
     """Per-step unit counts and algorithmic HBM bytes."""
     B, H, W = w.batch, w.H, w.W
@@ -126,7 +155,7 @@ def run_reference(args, w, rank):
         "config": {"workload": w.name, "note": w.note, "variant": w.variant, "n_sweeps": w.n_sweeps,
                    "step": f"bounded sample: {sample}"},
         "window_projections_per_s": value * nums["windows_per_sweep"],
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, **cpu_info()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -151,6 +180,12 @@ def run_gpu(args, w, rank, world):
     sched = {"auto": smre.SMRE_SCHED_AUTO, "graph": smre.SMRE_SCHED_GRAPH,
              "persistent": smre.SMRE_SCHED_PERSISTENT, "conveyor": smre.SMRE_SCHED_PERSISTENT,
              "strips": smre.SMRE_SCHED_STRIPS}[args.schedule]
+    # N > 1: a stack of frames is split by frame (no collective; outputs stay on their rank), a single image is
+    # replicated
+    from paper_1503_03492_b200.replicas import shard_workload
+    y_part, first_frame, frames_in_job, scaling = shard_workload(w.y, rank, world)
+    frames_total = w.batch
+    w.y = y_part
     nums = workload_numbers(w)
     sol = smre.Solver(w.H, w.W, w.sides, w.c, w.variant, w.batch, sched)
     stream = torch.cuda.Stream()
@@ -170,8 +205,14 @@ def run_gpu(args, w, rank, world):
             dist.barrier()
         torch.cuda.synchronize()
 
+    done = torch.zeros(max(w.batch, 1), dtype=torch.int32, device="cuda")
+
     def step_device():
-        smre.smre_project(sol.handle, y.data_ptr(), out.data_ptr(), w.n_sweeps, stream.cuda_stream)
+        if args.tol is not None:
+            smre.smre_project_tol(sol.handle, y.data_ptr(), out.data_ptr(), w.n_sweeps, args.tol, done.data_ptr(),
+                                  stream.cuda_stream)
+        else:
+            smre.smre_project(sol.handle, y.data_ptr(), out.data_ptr(), w.n_sweeps, stream.cuda_stream)
 
     def step_host():
         smre.smre_project_host(sol.handle, y_pin.data_ptr(), out_pin.data_ptr(), w.n_sweeps, stream.cuda_stream)
@@ -213,14 +254,20 @@ def run_gpu(args, w, rank, world):
         return _max_over_ranks(v, dist, "cuda")
 
     dev, dev_e, wall_e = max_over_ranks(dev), max_over_ranks(dev_e), max_over_ranks(wall_e)
-    sweeps_total = w.n_sweeps * args.steps * world
+    # whole job: replicas multiply the work, frame shards split it (the metric counts sweeps of the job's call)
+    sweeps_per_call = w.n_sweeps
+    if args.tol is not None:                  # what the stop rule actually ran (the slowest frame / tile)
+        torch.cuda.synchronize()
+        sweeps_per_call = int(done.cpu().numpy()[:max(w.batch, 1) if w.variant == "standard" else 1].max())
+    sweeps_total = sweeps_per_call * args.steps * (world if scaling == "weak" else 1)
     value = sweeps_total / dev
     e2e_value = sweeps_total / wall_e          # host-call wall time: the call blocks until the D2H copy is done
 
     if rank == 0:
         peak, peak_src, _ = measured_peaks()
         per_launch_s = dev / args.steps                       # persistent: one kernel = one step
-        kernel = "conveyor_kernel" if launch[0] == smre.SMRE_SCHED_PERSISTENT else "family_pass_kernel"
+        kernel = {smre.SMRE_SCHED_PERSISTENT: "conveyor_kernel", smre.SMRE_SCHED_STRIPS: "strips_kernel"}.get(
+            launch[0], "family_pass_kernel")
         if w.variant != "standard":
             kernel = "icd_shift_kernel"
         achieved = nums["bytes_per_step"] / per_launch_s / 1e9
@@ -229,49 +276,64 @@ def run_gpu(args, w, rank, world):
                     "algorithmic_bytes_per_step": nums["bytes_per_step"],
                     "note": "achieved = dense-model bytes of one whole step (all launches of the step) / "
                             "CUDA-event time of the step; see DESIGN.md sec. 7"}
-        if w.variant == "standard" and launch[0] == smre.SMRE_SCHED_PERSISTENT and w.name.startswith("C1") \
-                and w.n_sweeps == 200:
-            # dram__bytes_read.sum + dram__bytes_write.sum of this launch from the committed ncu --set full
-            # capture (profiles/r01_ncu_full_conveyor_c1_metrics.txt): 41.626 GB + 42.328 GB
-            roofline["traffic"] = 83.954e9
-            roofline["traffic_source"] = "profiles/r01_ncu_full_conveyor_c1_metrics.txt"
+        if w.variant == "standard" and launch[0] == smre.SMRE_SCHED_STRIPS and w.n_sweeps == 200 and args.tol is None:
+            # dram__bytes_read.sum + dram__bytes_write.sum of this launch, from the committed ncu --set full capture of
+            # the same command; the kernel skips stores that would not change memory, so the dense-model fraction
+            # (frac) and the fraction of the bytes actually moved (achieved_dram_frac) are both given
+            t, src = profile_metric(w.name, "dram_bytes_per_launch")
+            roofline["traffic"] = t
+            roofline["traffic_source"] = src
+            if t:
+                roofline["achieved_dram_frac"] = t / per_launch_s / 1e9 / peak
         if w.variant != "standard":
-            # ICD keeps q in registers: it is bound by fp32 issue, not by HBM.  Model: 5 fp32
-            # lane-instructions (add, fma, mul, sub, select) per pixel per level pass per inner cycle.
+            # ICD keeps q in registers: it is bound by instruction issue, not by HBM.  Numerator:
+            # thread-instructions the shift kernels EXECUTE per call (ncu smsp__thread_inst_executed.sum of the
+            # committed capture of this workload), not a model; peak = 148 SMs x 128 lanes x sm_max_mhz.
             _, _, sm_max = measured_peaks()
-            lane_instr = 5.0 * w.n_sweeps * nums["families"] * w.batch * w.H * w.W
+            lane_instr, src = profile_metric(w.name, "thread_inst_per_call")
             peak_alu = 148 * 128 * sm_max * 1e6
-            roofline = {"bound": "alu", "achieved": lane_instr / per_launch_s / 1e12, "peak": peak_alu / 1e12,
-                        "unit": "T lane-instr/s", "frac": lane_instr / per_launch_s / peak_alu, "traffic": None,
-                        "kernel": kernel, "hbm_frac": achieved / peak,
-                        "note": "fp32 issue model: 5 lane-instructions per pixel per level pass per cycle; peak = "
-                                "148 SMs x 128 lanes x sm_max_mhz; hbm_frac is reported so that nobody reads ICD "
-                                "as a bandwidth result"}
+            roofline = {"bound": "alu", "achieved": (lane_instr / per_launch_s / 1e12) if lane_instr else None,
+                        "peak": peak_alu / 1e12, "unit": "T lane-instr/s",
+                        "frac": (lane_instr / per_launch_s / peak_alu) if lane_instr else None, "traffic": None,
+                        "kernel": kernel, "hbm_frac": achieved / peak, "thread_inst_per_call": lane_instr,
+                        "thread_inst_source": src,
+                        "note": "executed thread-instructions per call (ncu) / time; peak = 148 SMs x 128 lanes x "
+                                "sm_max_mhz; hbm_frac is reported so that nobody reads ICD as a bandwidth result"}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             sample_sweeps = max(1, min(w.n_sweeps, args.ref_sweeps))
             v, dt, sample = time_oracle(w, sample_sweeps)
             cpu = {"value": v / w.batch, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-                   "seconds": dt}
+                   "seconds": dt, **cpu_info()}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev / args.steps * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "scaling": scaling, "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "note": w.note, "variant": w.variant, "n_sweeps": w.n_sweeps,
-                       "H": w.H, "W": w.W, "batch": w.batch, "families": nums["families"],
+                       "H": w.H, "W": w.W, "batch": frames_total, "frames_per_rank": w.batch,
+                       "families": nums["families"],
                        "windows_per_sweep": nums["windows_per_sweep"],
                        "schedule": ("icd_shifts" if w.variant != "standard" else {1: "graph", 2: "conveyor", 3: "strips"}.get(launch[0], str(launch[0]))),
                        "tiles": [launch[2], launch[3]],
                        "l2": ("q planes (204 MiB for C1, > 126 MB L2) are rewritten by every step: nothing of a step survives "
                               "in L2 for the next one") if flush is None else "256 MiB flush between steps",
-                       "parallelism": "replicas only" if world > 1 else "1 GPU"},
-            "window_projections_per_s": value * nums["windows_per_sweep"],
+                       "parallelism": ("1 GPU" if world == 1 else
+                                       "frames sharded over ranks, no collective" if scaling == "strong" else "replicas only")},
+            "window_projections_per_s": value * nums["windows_per_sweep"] * (world if scaling == "strong" else 1),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(y_pin.numel() * 4),
                     "d2h_bytes_per_step": int(out_pin.numel() * 4), "ms_per_step": wall_e / args.steps * 1e3},
             "gpu_launches": int(launch[1]) * args.steps,
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
             "wall_ms_per_step": wall / args.steps * 1e3,
         }
+        if args.tol is not None:
+            dn = done.cpu().numpy()
+            line["roofline"] = None           # the byte / instruction models above assume a fixed count
+            line["config"]["stop_rule"] = {"tol": args.tol, "max_sweeps": w.n_sweeps,
+                                           "iterations_done": [int(v) for v in (dn[:w.batch] if w.variant == "standard" else dn[:1])],
+                                           "note": "smre_project_tol: Alg. 2 / Listing 3 stop rule decided on the device; value "
+                                                   "counts the iterations of the slowest frame / tile; ms_per_step is the "
+                                                   "time to convergence; e2e is the fixed-count host call and does not apply"}
         print(json.dumps(line), flush=True)
     sol.close()
     if dist is not None:
@@ -290,6 +352,8 @@ def main():
     ap.add_argument("--schedule", default="auto", choices=["auto", "graph", "persistent", "conveyor", "strips"])
     ap.add_argument("--ref-sweeps", type=int, default=200, help="oracle sample size in sweeps (~12 s on C1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tol", type=float, default=None,
+                    help="run smre_project_tol with this tolerance (n_sweeps = max) and report the iterations done")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))

@@ -1009,6 +1009,7 @@ StripPlan *strips_plan_create(int H, int W, int B, int Wq, const int *sides, con
     }
     p->F = F;
     p->threads = (p->NWC + 2) * 32;                               // compute warps + waiter + issuer
+    // two builds: up to 18 warps with 96 registers, else 64 (measured on C1, 21 warps: 64 and 88 registers run alike)
     const bool big = p->threads > 576;
     if (Wq == 512) p->kernel = big ? kernel_ptr<512, 1024>() : kernel_ptr<512, 576>();
     else p->kernel = big ? kernel_ptr<0, 1024>() : kernel_ptr<0, 576>();

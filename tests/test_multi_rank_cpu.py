@@ -29,11 +29,19 @@ _WORKER = r"""
 import os, sys
 sys.path.insert(0, {root!r})
 import torch.distributed as dist
-from paper_1503_03492_b200.replicas import frame_shard, max_over_ranks, whole_job_value
+import numpy as np
+from paper_1503_03492_b200.replicas import frame_shard, max_over_ranks, shard_workload, whole_job_value
 dist.init_process_group("gloo")
 r, w = dist.get_rank(), dist.get_world_size()
 t = max_over_ranks(1.0 + r, dist)                 # rank 1 is the slow one
 s, n = frame_shard(7, r, w)
+# the code path bench.py uses: a stack shards by frame, a single image is replicated
+stack = np.arange(7 * 2 * 3, dtype=np.float32).reshape(7, 2, 3)
+part, first, total, scaling = shard_workload(stack, r, w)
+np.save(os.path.join({out!r}, "part%d.npy" % r), part)
+one, _, total1, scaling1 = shard_workload(stack[0], r, w)
+assert scaling == "strong" and total == 7 and first == s and part.shape[0] == n
+assert scaling1 == "weak" and total1 == w and one.shape == (2, 3)
 dist.barrier()
 open(os.path.join({out!r}, "rank%d.txt" % r), "w").write(" ".join(map(str, (r, w, t, s, n, whole_job_value(10.0, w, t)))))
 dist.destroy_process_group()
@@ -55,6 +63,10 @@ def test_gloo_world_size_2_max_over_ranks(tmp_path):
         assert float(row[2]) == 2.0                   # the max over ranks, on every rank
         assert float(row[5]) == 10.0                  # 2 ranks * 10 units / 2 s
     assert [(int(r[3]), int(r[4])) for r in rows] == [(0, 4), (4, 3)]
+    # the two ranks' shards, concatenated, are the whole stack
+    import numpy as np
+    parts = [np.load(tmp_path / f"part{r}.npy") for r in range(2)]
+    assert np.array_equal(np.concatenate(parts), np.arange(7 * 2 * 3, dtype=np.float32).reshape(7, 2, 3))
 
 
 def test_reference_arm_prints_on_rank_0_only():
