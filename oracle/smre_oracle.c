@@ -442,3 +442,74 @@ int smre_oracle_icd_tol(const double *y, int H, int W, const int *sides, const d
     }
     return smre_oracle_icd_levels_tol(y, H, W, K, level_c, max_cycles, tol, x_out, cycles_total, cycles_max);
 }
+
+/* ===========================================================================
+ * Threshold calibration (sec. 2.1, lines 89-113).
+ *
+ *   t_s(eps) = sum_{i in s} eps_i^2
+ *   (t_s)^(1/4) ~ N(mu_s = (|s| - 0.5)^(1/4), sigma_s^2 = 1 / (8 sqrt|s|))
+ *   Q_Omega = max_{s in Omega} ((t_s)^(1/4) - mu_s) / sigma_s
+ *   c_s(alpha) = 1 / (q_alpha sigma_s + mu_s)^4,  q_alpha the alpha quantile of Q_Omega
+ * Omega = the exact method's window set: every square window of every side in
+ * sides[] at every shift, fully inside the image (reading A6);
+ * |s| = side^2.  In this library's threshold convention c_S = 1 / c_s(alpha)
+ * = (q_alpha sigma_s + mu_s)^4.
+ * Readings (DESIGN.md A-CAL): the noise images are INPUTS (unit variance); the
+ * alpha quantile of the n simulated values is the order statistic of rank
+ * ceil(alpha n) (1-based, clamped to [1, n]).
+ * ------------------------------------------------------------------------- */
+double smre_oracle_cal_mu(int side)    { double n = (double)side * side; return pow(n - 0.5, 0.25); }
+double smre_oracle_cal_sigma(int side) { double n = (double)side * side; return sqrt(1.0 / (8.0 * sqrt(n))); }
+
+/* Q_Omega of one image. */
+int smre_oracle_q_stat(const double *eps, int H, int W, const int *sides, int n_sides, double *q_out)
+{
+    if (!eps || !sides || !q_out || H <= 0 || W <= 0 || n_sides <= 0) return -1;
+    double best = -HUGE_VAL;
+    for (int a = 0; a < n_sides; ++a) {
+        const int s = sides[a];
+        if (s < 1 || s > H || s > W) return -1;
+        const double mu = smre_oracle_cal_mu(s), sg = smre_oracle_cal_sigma(s);
+        for (int wy = 0; wy + s <= H; ++wy)
+            for (int wx = 0; wx + s <= W; ++wx) {
+                double t = 0.0;
+                for (int r = wy; r < wy + s; ++r)
+                    for (int col = wx; col < wx + s; ++col) {
+                        double v = eps[(size_t)r * W + col];
+                        t += v * v;
+                    }
+                double z = (pow(t, 0.25) - mu) / sg;
+                if (z > best) best = z;
+            }
+    }
+    *q_out = best;
+    return 0;
+}
+
+static int cmp_double(const void *a, const void *b)
+{
+    double x = *(const double *)a, y = *(const double *)b;
+    return (x > y) - (x < y);
+}
+
+/* q_alpha = order statistic of rank ceil(alpha n) of q[0..n), then c_out[a] = (q_alpha sigma + mu)^4. */
+int smre_oracle_thresholds_from_q(const double *q, int n, double alpha, const int *sides, int n_sides,
+                                  double *q_alpha_out, double *c_out)
+{
+    if (!q || n <= 0 || !sides || n_sides <= 0 || !c_out || !(alpha > 0.0) || !(alpha <= 1.0)) return -1;
+    double *tmp = (double *)malloc(sizeof(double) * (size_t)n);
+    if (!tmp) return -1;
+    memcpy(tmp, q, sizeof(double) * (size_t)n);
+    qsort(tmp, (size_t)n, sizeof(double), cmp_double);
+    int k = (int)ceil(alpha * (double)n);
+    if (k < 1) k = 1;
+    if (k > n) k = n;
+    const double qa = tmp[k - 1];
+    free(tmp);
+    if (q_alpha_out) *q_alpha_out = qa;
+    for (int a = 0; a < n_sides; ++a) {
+        double base = qa * smre_oracle_cal_sigma(sides[a]) + smre_oracle_cal_mu(sides[a]);
+        c_out[a] = base * base * base * base;
+    }
+    return 0;
+}

@@ -76,6 +76,10 @@ def _load():
         lib.smre_oracle_icd_levels_replay.argtypes = [
             _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_int, ctypes.c_double, _ip,
             ctypes.c_double, _dp, ctypes.POINTER(ctypes.c_longlong)]
+        lib.smre_oracle_q_stat.restype = ctypes.c_int
+        lib.smre_oracle_q_stat.argtypes = [_dp, ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, _dp]
+        lib.smre_oracle_thresholds_from_q.restype = ctypes.c_int
+        lib.smre_oracle_thresholds_from_q.argtypes = [_dp, ctypes.c_int, ctypes.c_double, _ip, ctypes.c_int, _dp, _dp]
         lib.smre_oracle_window_sums.restype = ctypes.c_int
         lib.smre_oracle_window_sums.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
         _lib = lib
@@ -263,6 +267,31 @@ def replay_icd(y, sides, c, max_cycles, tol, tile_cycles, band):
                                              _p(counts, _ip), float(band), _p(x, _dp), ctypes.byref(bad)),
            "smre_oracle_icd_levels_replay")
     return x, bad.value
+
+
+def q_stat(eps, sides):
+    """Q_Omega of one image [H,W], or of every frame of a stack [n,H,W] -> array [n]."""
+    lib = _load()
+    eps = _f64(eps)
+    sides = _i32(sides)
+    if eps.ndim == 3:
+        return np.array([q_stat(f, sides) for f in eps])
+    H, W = eps.shape
+    q = ctypes.c_double(0.0)
+    _check(lib.smre_oracle_q_stat(_p(eps, _dp), H, W, _p(sides, _ip), len(sides), ctypes.byref(q)), "smre_oracle_q_stat")
+    return q.value
+
+
+def thresholds_from_q(q, alpha, sides):
+    """(q_alpha, thresholds c_S = (q_alpha sigma_s + mu_s)^4 per side) from simulated Q values."""
+    lib = _load()
+    q = _f64(q).ravel()
+    sides = _i32(sides)
+    c = np.zeros(len(sides), np.float64)
+    qa = ctypes.c_double(0.0)
+    _check(lib.smre_oracle_thresholds_from_q(_p(q, _dp), len(q), float(alpha), _p(sides, _ip), len(sides),
+                                             ctypes.byref(qa), _p(c, _dp)), "smre_oracle_thresholds_from_q")
+    return qa.value, c
 
 
 def project(y, sides, c, n_sweeps, variant):
