@@ -185,6 +185,26 @@ smre_status smre_plan_check(int H, int W, const int *sides, int n_sides, int n_s
 smre_status smre_project_noalloc(int H, int W, const int *sides, int n_sides, const float *c_table,
                                  const float *y_dev, float *x_out_dev, int n_sweeps, void *cuda_stream);
 
+/* ---- threshold calibration (sec. 2.1) ---------------------------------------------------- */
+
+/*
+ * The thresholds that balance the multi-scale test, from simulated noise.  noise_dev: DEVICE,
+ * n_frames images [n_frames][H][W] of unit-variance noise drawn by the caller (the library draws no random numbers).
+ * For every frame the extreme-value statistic
+ *     Q = max over every window s of every side in sides[], at every shift, fully inside the image, of
+ *         ((t_s)^(1/4) - mu_s) / sigma_s,   t_s = sum of squares over s,   mu_s = (|s| - 0.5)^(1/4),
+ *         sigma_s^2 = 1 / (8 sqrt|s|),   |s| = side^2
+ * is written to q_stat_dev (DEVICE, n_frames floats); q_alpha = the order statistic of rank ceil(alpha * n_frames)
+ * (alpha as passed, a float, the product in double; clamped to [1, n_frames]) of
+ * those values goes to q_alpha_dev (DEVICE, 1 float, may be NULL), and the THRESHOLD of every side,
+ *     c_S = 1 / c_s(alpha) = (q_alpha sigma_s + mu_s)^4
+ * to c_table_dev (DEVICE, n_sides floats, order of sides[]): the table smre_create takes.  sides: HOST, distinct,
+ * 1 <= side <= min(H, W, SMRE_MAX_SIDE).  0 < alpha <= 1.  fp32; the window sums add positive terms only.
+ * Asynchronous on cuda_stream; allocates nothing.
+ */
+smre_status smre_calibrate(int H, int W, int n_frames, const int *sides, int n_sides, const float *noise_dev,
+                           float alpha, float *q_stat_dev, float *q_alpha_dev, float *c_table_dev, void *cuda_stream);
+
 /* Text of the last error on the calling thread ("" if none).  Never NULL. */
 const char *smre_last_error(void);
 

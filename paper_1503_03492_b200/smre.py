@@ -21,7 +21,7 @@ _STATUS = {0: "SMRE_OK", 1: "SMRE_EINVAL", 2: "SMRE_EUNSUPPORTED", 3: "SMRE_ENOM
 exported_symbols = (
     "smre_create", "smre_project", "smre_project_host", "smre_destroy", "smre_set_schedule",
     "smre_info", "smre_family", "smre_export_increments", "smre_last_launch", "smre_last_error",
-    "smre_plan_check", "smre_project_noalloc", "smre_project_tol", "smre_export_tile_cycles",
+    "smre_plan_check", "smre_project_noalloc", "smre_project_tol", "smre_export_tile_cycles", "smre_calibrate",
 )
 
 
@@ -62,6 +62,8 @@ def load_library(build_if_missing: bool = True):
     lib.smre_plan_check.argtypes = [ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                     _ip, _ip, _ip, _ip, _llp]
     lib.smre_project_noalloc.argtypes = [ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, _fp, _vp, _vp, ctypes.c_int, _vp]
+    lib.smre_calibrate.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, _vp, ctypes.c_float,
+                                   _vp, _vp, _vp, _vp]
     lib.smre_project_tol.argtypes = [_vp, _vp, _vp, ctypes.c_int, ctypes.c_float, _vp, _vp]
     lib.smre_export_tile_cycles.argtypes = [_vp, ctypes.c_int, _vp, _ip, _ip, _vp]
     for name in exported_symbols:
@@ -126,6 +128,27 @@ def smre_export_tile_cycles(handle, shift, out_ptr=None, stream=0):
     ty, tx = ctypes.c_int(), ctypes.c_int()
     _check(load_library().smre_export_tile_cycles(handle, int(shift), out_ptr, ctypes.byref(ty), ctypes.byref(tx), stream))
     return ty.value, tx.value
+
+
+def smre_calibrate(H, W, n_frames, sides, noise_ptr, alpha, q_stat_ptr, q_alpha_ptr, c_table_ptr, stream=0):
+    """Thresholds from simulated noise (sec. 2.1); all *_ptr are device addresses."""
+    sides = np.ascontiguousarray(sides, dtype=np.int32)
+    _check(load_library().smre_calibrate(int(H), int(W), int(n_frames), sides.ctypes.data_as(_ip), len(sides), noise_ptr,
+                                         float(alpha), q_stat_ptr, q_alpha_ptr, c_table_ptr, stream))
+
+
+def calibrate(noise, sides, alpha):
+    """noise: float32 CUDA tensor [n,H,W] of unit-variance noise -> (c_table [n_sides], q_alpha [1], Q [n]) tensors."""
+    import torch
+    if not (noise.is_cuda and noise.dtype == torch.float32 and noise.is_contiguous() and noise.dim() == 3):
+        raise ValueError("noise must be a contiguous float32 CUDA tensor [n, H, W]")
+    n, H, W = noise.shape
+    q = torch.empty(n, dtype=torch.float32, device=noise.device)
+    qa = torch.empty(1, dtype=torch.float32, device=noise.device)
+    c = torch.empty(len(sides), dtype=torch.float32, device=noise.device)
+    smre_calibrate(H, W, n, sides, noise.data_ptr(), alpha, q.data_ptr(), qa.data_ptr(), c.data_ptr(),
+                   torch.cuda.current_stream(noise.device).cuda_stream)
+    return c, qa, q
 
 
 def smre_destroy(handle):
