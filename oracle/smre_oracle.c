@@ -513,3 +513,27 @@ int smre_oracle_thresholds_from_q(const double *q, int n, double alpha, const in
     }
     return 0;
 }
+
+/* ===========================================================================
+ * Second-order SOFI cumulant at zero time lag (Eq. 19):
+ *     C_2(r, 0) = <F^2(r, t)>_t - <F(r, t)>_t^2
+ * per pixel over the n frames of a stack F[n][H][W] (population variance: both means divide by n).
+ * The plain definition, two passes per pixel.
+ * ------------------------------------------------------------------------- */
+int smre_oracle_cumulant2(const double *stack, int n, int H, int W, double *c2_out)
+{
+    if (!stack || !c2_out || n <= 0 || H <= 0 || W <= 0) return -1;
+    size_t N = (size_t)H * W;
+    for (size_t i = 0; i < N; ++i) {
+        double m1 = 0.0, m2 = 0.0;
+        for (int t = 0; t < n; ++t) {
+            double v = stack[(size_t)t * N + i];
+            m1 += v;
+            m2 += v * v;
+        }
+        m1 /= (double)n;
+        m2 /= (double)n;
+        c2_out[i] = m2 - m1 * m1;
+    }
+    return 0;
+}

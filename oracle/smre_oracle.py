@@ -80,6 +80,8 @@ def _load():
         lib.smre_oracle_q_stat.argtypes = [_dp, ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, _dp]
         lib.smre_oracle_thresholds_from_q.restype = ctypes.c_int
         lib.smre_oracle_thresholds_from_q.argtypes = [_dp, ctypes.c_int, ctypes.c_double, _ip, ctypes.c_int, _dp, _dp]
+        lib.smre_oracle_cumulant2.restype = ctypes.c_int
+        lib.smre_oracle_cumulant2.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
         lib.smre_oracle_window_sums.restype = ctypes.c_int
         lib.smre_oracle_window_sums.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
         _lib = lib
@@ -292,6 +294,16 @@ def thresholds_from_q(q, alpha, sides):
     _check(lib.smre_oracle_thresholds_from_q(_p(q, _dp), len(q), float(alpha), _p(sides, _ip), len(sides),
                                              ctypes.byref(qa), _p(c, _dp)), "smre_oracle_thresholds_from_q")
     return qa.value, c
+
+
+def cumulant2(stack):
+    """C_2(r, 0) = <F^2>_t - <F>_t^2 per pixel of a stack [n,H,W] (Eq. 19)."""
+    lib = _load()
+    stack = _f64(stack)
+    n, H, W = stack.shape
+    out = np.empty((H, W), np.float64)
+    _check(lib.smre_oracle_cumulant2(_p(stack, _dp), n, H, W, _p(out, _dp)), "smre_oracle_cumulant2")
+    return out
 
 
 def project(y, sides, c, n_sweeps, variant):

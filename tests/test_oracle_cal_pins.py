@@ -92,3 +92,25 @@ def test_fourth_root_transform_statistics(oracle):
     qa, c = oracle.thresholds_from_q(Q, 0.8, sides)
     fresh = oracle.q_stat(rng.standard_normal((200, 24, 24)), sides)
     assert 0.65 < (fresh <= qa).mean() < 0.92
+
+
+# ---- second-order SOFI cumulant (Eq. 19) --------------------------------------------------
+def test_cumulant2_closed_forms(oracle):
+    rng = np.random.default_rng(12)
+    # a constant pixel has no fluctuation; a pixel that blinks between a and b half of the time has ((a - b) / 2)^2
+    n, H, W = 8, 3, 4
+    s = np.full((n, H, W), 2.5)
+    s[::2, 1, 2] = 7.0
+    s[1::2, 1, 2] = 1.0
+    c2 = oracle.cumulant2(s)
+    want = np.zeros((H, W))
+    want[1, 2] = 9.0
+    np.testing.assert_allclose(c2, want, atol=1e-13)
+    # the population variance of numpy, shift invariance (cumulants of order >= 2 ignore a constant background) and
+    # the quadratic scaling with the brightness
+    s = rng.standard_normal((50, 6, 5)) * rng.uniform(0.5, 2.0, (1, 6, 5)) + 3.0
+    c2 = oracle.cumulant2(s)
+    np.testing.assert_allclose(c2, s.var(axis=0), rtol=1e-12)
+    np.testing.assert_allclose(oracle.cumulant2(s + 100.0), c2, rtol=1e-9)
+    np.testing.assert_allclose(oracle.cumulant2(3.0 * s), 9.0 * c2, rtol=1e-12)
+    assert (c2 >= 0).all()
