@@ -205,6 +205,14 @@ smre_status smre_project_noalloc(int H, int W, const int *sides, int n_sides, co
 smre_status smre_calibrate(int H, int W, int n_frames, const int *sides, int n_sides, const float *noise_dev,
                            float alpha, float *q_stat_dev, float *q_alpha_dev, float *c_table_dev, void *cuda_stream);
 
+/*
+ * Second-order SOFI cumulant at zero time lag (Eq. 19): C_2 = <F^2>_t - <F>_t^2 per pixel over the
+ * n_frames frames of stack_dev (DEVICE, [n_frames][H][W] fp32, 16-byte aligned), e.g. the projected frames of a
+ * batched smre_project; both means divide by n_frames.  c2_out_dev: DEVICE, H*W fp32, 16-byte aligned.
+ * Asynchronous on cuda_stream; allocates nothing.
+ */
+smre_status smre_cumulant2(int H, int W, int n_frames, const float *stack_dev, float *c2_out_dev, void *cuda_stream);
+
 /* Text of the last error on the calling thread ("" if none).  Never NULL. */
 const char *smre_last_error(void);
 

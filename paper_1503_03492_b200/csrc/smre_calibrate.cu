@@ -17,6 +17,7 @@
 #include "smre_common.cuh"
 
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 
 namespace smre {
@@ -170,6 +171,68 @@ extern "C" smre_status smre_calibrate(int H, int W, int n_frames, const int *sid
     quantile_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<unsigned *>(q_stat_dev), n_frames, k, cs, list, q_alpha_dev,
                                         c_table_dev);
     e = cudaGetLastError();
+    if (e != cudaSuccess) return cal_fail(SMRE_ECUDA, cudaGetErrorString(e));
+    return SMRE_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Second-order SOFI cumulant at zero time lag (Eq. 19):
+//     C_2(r, 0) = <F^2(r, t)>_t - <F(r, t)>_t^2     per pixel over the n frames of a stack (e.g. the projected frames).
+// HBM-bound: every frame is read once, coalesced (thread = 4 consecutive pixels, float4), the frame loop is unrolled
+// for loads in flight.  The two moments are accumulated around the FIRST frame's value of the pixel (a shift leaves
+// a cumulant of order >= 2 unchanged, and it removes the cancellation of <F^2> - <F>^2 on a bright background).
+namespace smre {
+
+__global__ void __launch_bounds__(256)
+cumulant2_kernel(const float *__restrict__ stack, int n, long long N, float *__restrict__ c2)
+{
+    const long long i4 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (i4 >= N) return;
+    const float inv_n = 1.0f / (float)n;
+    if (i4 + 4 <= N && (N & 3) == 0) {
+        const float4 ref = *reinterpret_cast<const float4 *>(stack + i4);
+        float4 s1 = make_float4(0.f, 0.f, 0.f, 0.f), s2 = s1;
+#pragma unroll 4
+        for (int t = 1; t < n; ++t) {
+            const float4 v = __ldcs(reinterpret_cast<const float4 *>(stack + (long long)t * N + i4));
+            const float dx = v.x - ref.x, dy = v.y - ref.y, dz = v.z - ref.z, dw = v.w - ref.w;
+            s1.x += dx; s1.y += dy; s1.z += dz; s1.w += dw;
+            s2.x = fmaf(dx, dx, s2.x); s2.y = fmaf(dy, dy, s2.y); s2.z = fmaf(dz, dz, s2.z); s2.w = fmaf(dw, dw, s2.w);
+        }
+        float4 o;
+        o.x = fmaf(-(s1.x * inv_n), s1.x * inv_n, s2.x * inv_n);
+        o.y = fmaf(-(s1.y * inv_n), s1.y * inv_n, s2.y * inv_n);
+        o.z = fmaf(-(s1.z * inv_n), s1.z * inv_n, s2.z * inv_n);
+        o.w = fmaf(-(s1.w * inv_n), s1.w * inv_n, s2.w * inv_n);
+        *reinterpret_cast<float4 *>(c2 + i4) = o;
+    } else {
+        for (long long i = i4; i < min(i4 + 4, N); ++i) {
+            const float ref = stack[i];
+            float s1 = 0.f, s2 = 0.f;
+            for (int t = 1; t < n; ++t) {
+                const float d = stack[(long long)t * N + i] - ref;
+                s1 += d;
+                s2 = fmaf(d, d, s2);
+            }
+            c2[i] = fmaf(-(s1 * inv_n), s1 * inv_n, s2 * inv_n);
+        }
+    }
+}
+
+}  // namespace smre
+
+extern "C" smre_status smre_cumulant2(int H, int W, int n_frames, const float *stack_dev, float *c2_out_dev,
+                                      void *cuda_stream)
+{
+    if (!stack_dev || !c2_out_dev) return cal_fail(SMRE_EINVAL, "smre_cumulant2: NULL argument");
+    if (H <= 0 || W <= 0 || n_frames <= 0) return cal_fail(SMRE_EINVAL, "smre_cumulant2: H, W, n_frames must be positive");
+    if (((uintptr_t)stack_dev & 15) || ((uintptr_t)c2_out_dev & 15))
+        return cal_fail(SMRE_EINVAL, "smre_cumulant2: pointers must be 16-byte aligned");
+    const long long N = (long long)H * W;
+    const long long threads = (N + 3) / 4;
+    cumulant2_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(stack_dev, n_frames, N,
+                                                                                           c2_out_dev);
+    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cal_fail(SMRE_ECUDA, cudaGetErrorString(e));
     return SMRE_OK;
 }

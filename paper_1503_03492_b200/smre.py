@@ -21,7 +21,7 @@ _STATUS = {0: "SMRE_OK", 1: "SMRE_EINVAL", 2: "SMRE_EUNSUPPORTED", 3: "SMRE_ENOM
 exported_symbols = (
     "smre_create", "smre_project", "smre_project_host", "smre_destroy", "smre_set_schedule",
     "smre_info", "smre_family", "smre_export_increments", "smre_last_launch", "smre_last_error",
-    "smre_plan_check", "smre_project_noalloc", "smre_project_tol", "smre_export_tile_cycles", "smre_calibrate",
+    "smre_plan_check", "smre_project_noalloc", "smre_project_tol", "smre_export_tile_cycles", "smre_calibrate", "smre_cumulant2",
 )
 
 
@@ -64,6 +64,7 @@ def load_library(build_if_missing: bool = True):
     lib.smre_project_noalloc.argtypes = [ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, _fp, _vp, _vp, ctypes.c_int, _vp]
     lib.smre_calibrate.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int, _vp, ctypes.c_float,
                                    _vp, _vp, _vp, _vp]
+    lib.smre_cumulant2.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]
     lib.smre_project_tol.argtypes = [_vp, _vp, _vp, ctypes.c_int, ctypes.c_float, _vp, _vp]
     lib.smre_export_tile_cycles.argtypes = [_vp, ctypes.c_int, _vp, _ip, _ip, _vp]
     for name in exported_symbols:
@@ -149,6 +150,22 @@ def calibrate(noise, sides, alpha):
     smre_calibrate(H, W, n, sides, noise.data_ptr(), alpha, q.data_ptr(), qa.data_ptr(), c.data_ptr(),
                    torch.cuda.current_stream(noise.device).cuda_stream)
     return c, qa, q
+
+
+def smre_cumulant2(H, W, n_frames, stack_ptr, out_ptr, stream=0):
+    """C_2 = <F^2> - <F>^2 per pixel over a stack (Eq. 19); device addresses."""
+    _check(load_library().smre_cumulant2(int(H), int(W), int(n_frames), stack_ptr, out_ptr, stream))
+
+
+def cumulant2(stack):
+    """stack: float32 CUDA tensor [n,H,W] -> float32 tensor [H,W]."""
+    import torch
+    if not (stack.is_cuda and stack.dtype == torch.float32 and stack.is_contiguous() and stack.dim() == 3):
+        raise ValueError("stack must be a contiguous float32 CUDA tensor [n, H, W]")
+    n, H, W = stack.shape
+    out = torch.empty((H, W), dtype=torch.float32, device=stack.device)
+    smre_cumulant2(H, W, n, stack.data_ptr(), out.data_ptr(), torch.cuda.current_stream(stack.device).cuda_stream)
+    return out
 
 
 def smre_destroy(handle):

@@ -14,7 +14,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def test_library_builds_and_exports_header_symbols():
     lib = smre.load_library()
     header = open(os.path.join(ROOT, "include", "smre.h")).read()
-    declared = set(re.findall(r"\b(smre_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(smre_[a-z_0-9]+)\s*\(", header))
     assert declared == set(smre.exported_symbols)
     for name in declared:
         assert getattr(lib, name) is not None

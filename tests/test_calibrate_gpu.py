@@ -80,3 +80,18 @@ def test_calibrate_errors():
         assert e.value.status == smre.smre.SMRE_EINVAL
     with pytest.raises(smre.SmreError):
         smre.smre_calibrate(8, 8, 2, [1], None, 0.5, out.data_ptr(), out.data_ptr(), out.data_ptr())
+
+
+@pytest.mark.parametrize("n,H,W", [(64, 256, 256), (7, 33, 35), (2, 5, 4), (1, 16, 16)])
+def test_cumulant2_matches_oracle(oracle, n, H, W):
+    """Eq. 19 on a SOFI-like stack: bright background, blinking emitters."""
+    rng = np.random.default_rng(n + W)
+    stack = (200.0 + 3.0 * rng.standard_normal((n, H, W))).astype(np.float32)
+    stack[:, H // 2, W // 2] += (40.0 * (rng.random(n) < 0.5)).astype(np.float32)      # a blinking emitter
+    c2 = smre.cumulant2(torch.from_numpy(stack).cuda())
+    torch.cuda.synchronize()
+    ref = oracle.cumulant2(stack)
+    # fp32 moments about the first frame: deviations ~ 10, n terms -> relative 1e-5 of the variance scale is ample
+    assert np.abs(c2.cpu().numpy() - ref).max() <= 2e-5 * max(1.0, float(ref.max()))
+    if n > 1:
+        assert ref[H // 2, W // 2] > 5 * np.median(ref) or n < 4
