@@ -282,8 +282,11 @@ struct ComputeState {
 #endif
     int pos = 0;                        // q ring: next free row
     unsigned mc = 0;                    // transitions done
-    unsigned seen_m3, seen_m2, seen_m1, seen_p1, seen_p2, seen_p3;   // cached progress words of the strips around
-                                                                     // (flow control of their mailbox rings)
+    float *tcol;                        // my column of the tile, addressed by image row: tcol[y * pitch]
+    unsigned long long *box0;           // my column of slot 0 of my mailbox, addressed the same way
+    long long slot_words, dest_step;    // next slot of my mailbox; same slot of the next strip's mailbox
+    unsigned *seen_sh;                  // shared memory [6]: cached progress words of strips j-3..j-1, j+1..j+3
+                                        // (flow control of their mailbox rings)
 };
 
 // Mailbox slot of transition number mc in the mailbox of the strip of CTA `cta`, addressed by image row / column:
@@ -323,7 +326,8 @@ __device__ __forceinline__ void transition(const StripArgs &A, float *tile, int 
 {
     constexpr int MAXR = 8;                                    // rows requested at once
     static_assert(ST_HOPS == 3, "the sends below are written out for three hops");
-    const int NS = A.NS, Wq = A.Wq, T = A.T;
+    static_assert((ST_RING & (ST_RING - 1)) == 0, "ST_RING must be a power of two");
+    const int NS = A.NS;
     const unsigned mc = ++cs.mc;
     const unsigned tag = A.tag_base + mc;
     if (ST_KO(A, 1)) { bar_sync(2, NT); return; }
@@ -332,81 +336,73 @@ __device__ __forceinline__ void transition(const StripArgs &A, float *tile, int 
     cs.t_macro += c0 - cs.t_last;
 #endif
     const bool mine = tid < A.W;
-    float *tcol = tile + (T / 2 - j * T) * pitch + tid;         // tcol[y * pitch]: image row y, my column
-    unsigned long long *box = st_mailbox(A, cta, j, mc) + tid;
-    const long long dest_step = st_dest_step(A);
+    float *const tcol = cs.tcol;                                // tcol[y * pitch]: image row y, my column
+    unsigned long long *const box = cs.box0 + (size_t)(mc & (ST_RING - 1)) * cs.slot_words;   // box[y * pitch]
+    const long long dest_step = cs.dest_step;
 
-    // progress of the strips around, for the flow control of the NEXT transition: requested now, used at the end
-    const int up1 = j >= 1, up2 = j >= 2 ? 2 : up1, up3 = j >= 3 ? 3 : up2;
-    const int dn1 = j + 1 < NS, dn2 = j + 2 < NS ? 2 : dn1, dn3 = j + 3 < NS ? 3 : dn2;
-    const unsigned s_m1 = ld_relaxed_gpu32(A.done + (size_t)(cta - up1) * 32);
-    const unsigned s_p1 = ld_relaxed_gpu32(A.done + (size_t)(cta + dn1) * 32);
-    const unsigned s_m2 = ld_relaxed_gpu32(A.done + (size_t)(cta - up2) * 32);
-    const unsigned s_p2 = ld_relaxed_gpu32(A.done + (size_t)(cta + dn2) * 32);
-    const unsigned s_m3 = ld_relaxed_gpu32(A.done + (size_t)(cta - up3) * 32);
-    const unsigned s_p3 = ld_relaxed_gpu32(A.done + (size_t)(cta + dn3) * 32);
-
-    // departures
-    auto send = [&](int d, int lo, int hi, unsigned &seen) {
+    // departures first: they are what the strips around are waiting for
+    auto send = [&](int d, int lo, int hi, int k) {
         if (lo >= hi) return;
+        unsigned seen = *(volatile unsigned *)(cs.seen_sh + k);
         st_ring_space(A, cta, d, tag, mc, seen, w);
         if (!mine) return;
         unsigned long long *dst = box + d * dest_step;
         for (int y = lo; y < hi; ++y)
-            st_relaxed_gpu64(dst + y * Wq, pack_word(tag, tcol[y * pitch]));
+            st_relaxed_gpu64(dst + y * pitch, pack_word(tag, tcol[y * pitch]));
     };
-    send(-1, e.send_lo[2], e.send_hi[2], cs.seen_m1);
-    send(+1, e.send_lo[3], e.send_hi[3], cs.seen_p1);
-    send(-2, e.send_lo[1], e.send_hi[1], cs.seen_m2);
-    send(+2, e.send_lo[4], e.send_hi[4], cs.seen_p2);
-    send(-3, e.send_lo[0], e.send_hi[0], cs.seen_m3);
-    send(+3, e.send_lo[5], e.send_hi[5], cs.seen_p3);
+    send(-1, e.send_lo[2], e.send_hi[2], 2);
+    send(+1, e.send_lo[3], e.send_hi[3], 3);
+    send(-2, e.send_lo[1], e.send_hi[1], 1);
+    send(+2, e.send_lo[4], e.send_hi[4], 4);
+    send(-3, e.send_lo[0], e.send_hi[0], 0);
+    send(+3, e.send_lo[5], e.send_hi[5], 5);
 #ifdef SMRE_ST_KO
     const long long c1 = clock64();
 #endif
-    // arrivals: all words of a batch are requested at once, then re-requested until their tag is right
-    const int n0 = e.recv_hi[0] - e.recv_lo[0], n1 = e.recv_hi[1] - e.recv_lo[1];
-    if (mine && n0 + n1 > 0) {
+    // progress words of the strips around (flow control of the mailbox rings at the NEXT transitions): one thread per
+    // neighbour asks now and files the answer in shared memory after the arrivals
+    unsigned s_new = 0;
+    const int nd = tid < ST_HOPS ? tid - ST_HOPS : tid - ST_HOPS + 1;       // tid 0..5 -> strip j-3..j-1, j+1..j+3
+    const bool asks = tid < 2 * ST_HOPS && j + nd >= 0 && j + nd < NS;
+    if (asks) s_new = ld_relaxed_gpu32(A.done + (size_t)(cta + nd) * 32);
+
+    // arrivals: all words of a batch are requested at once; a word whose tag is right goes to the tile, the others
+    // are requested again.  The loop is kept short on purpose: with every compute warp in it, the time of one round
+    // is set by the instructions it issues, and an arrival is seen one round late on average.
+    const int n0 = e.recv_hi[0] - e.recv_lo[0], n = n0 + e.recv_hi[1] - e.recv_lo[1];
+    if (mine && n > 0) {
         w.begin();
-        for (int r0 = 0; r0 < n0 + n1; r0 += MAXR) {
-            int yy[MAXR];
-            unsigned long long wd[MAXR];
+        for (int r0 = 0; r0 < n; r0 += MAXR) {
+            int off[MAXR];
+            unsigned missing = 0;
 #pragma unroll
             for (int r = 0; r < MAXR; ++r) {
                 const int i = r0 + r;
-                yy[r] = i < n0 ? e.recv_lo[0] + i : i < n0 + n1 ? e.recv_lo[1] + (i - n0) : -1;
+                off[r] = (i < n0 ? e.recv_lo[0] + i : e.recv_lo[1] + (i - n0)) * pitch;
+                if (i < n) missing |= 1u << r;
             }
-            unsigned missing;
-            int tries = 0;
-            do {
-                if (tries++ && w.slow(ST_W_MAIL)) {
-#ifdef SMRE_ST_KO
-                    if (tid < 40 || (tid & 31) == 0)
-                        printf("MAIL timeout strip %d tid %d mc %u tag %u rows [%d,%d)+[%d,%d) missing %x got tags %u %u\n", j, tid, mc, tag,
-                               e.recv_lo[0], e.recv_hi[0], e.recv_lo[1], e.recv_hi[1], missing, (unsigned)(wd[0] >> 32), (unsigned)(wd[1] >> 32));
-#endif
-                    break;
-                }
+            for (;;) {
+                unsigned long long wd[MAXR];
 #pragma unroll
                 for (int r = 0; r < MAXR; ++r)
-                    if (yy[r] >= 0) wd[r] = ld_relaxed_gpu64(box + yy[r] * Wq);
-                missing = 0;
+                    if (missing >> r & 1u) wd[r] = ld_relaxed_gpu64(box + off[r]);
 #pragma unroll
                 for (int r = 0; r < MAXR; ++r)
-                    if (yy[r] >= 0 && (unsigned)(wd[r] >> 32) != tag) missing |= 1u << r;
+                    if ((missing >> r & 1u) && (unsigned)(wd[r] >> 32) == tag) {
+                        tcol[off[r]] = __uint_as_float((unsigned)wd[r]);
+                        missing &= ~(1u << r);
+                    }
                 if (ST_KO(A, 64)) missing = 0;
-            } while (missing);
-#pragma unroll
-            for (int r = 0; r < MAXR; ++r)
-                if (yy[r] >= 0) tcol[yy[r] * pitch] = __uint_as_float((unsigned)wd[r]);
+                if (!missing || w.slow(ST_W_MAIL)) break;
+            }
         }
     }
+    if (asks) *(volatile unsigned *)(cs.seen_sh + tid) = s_new;
 #ifdef SMRE_ST_KO
     const long long c2 = clock64();
 #endif
     bar_sync(2, NT);
     if (tid == 0) st_relaxed_gpu32(A.done + (size_t)cta * 32, tag);   // my mailbox slot of this transition is free again
-    cs.seen_m1 = s_m1; cs.seen_p1 = s_p1; cs.seen_m2 = s_m2; cs.seen_p2 = s_p2; cs.seen_m3 = s_m3; cs.seen_p3 = s_p3;
 #ifdef SMRE_ST_KO
     const long long c3 = clock64();
     cs.t_send += c1 - c0; cs.t_recv += c2 - c1; cs.t_bar += c3 - c2; cs.t_last = c3;
@@ -695,6 +691,7 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
     unsigned *allow = abort_flag + 2;                           // tol mode: sweeps the run is allowed to execute so far
     unsigned *stopped = abort_flag + 3;                         // tol mode: the stop rule has fired
     double *wsum = reinterpret_cast<double *>(abort_flag + 4);  // [ST_MAX_WARPS + 1] per-warp parts of ||x_r - x_{r-1}||^2
+    unsigned *seen_sh = reinterpret_cast<unsigned *>(wsum + ST_MAX_WARPS + 2);   // [2 * ST_HOPS], see transition()
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int NWC = A.NWC, NT = NWC * 32, NTL = NT + (ST_KO(A, 32) ? 0 : 32);
@@ -765,12 +762,17 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
         const float *yim = A.y + (size_t)frame * H * W;
         for (int y = tab[0].hold_lo; y < tab[0].hold_hi; ++y)
             for (int c = tid; c < W; c += NT) tile[(y + slot_base) * pitch + c] = yim[(size_t)y * W + c];
+        if (tid < 2 * ST_HOPS) seen_sh[tid] = A.tag_base;
         bar_sync(2, NT);
         ComputeState cs;
 #ifdef SMRE_ST_KO
         cs.t_last = clock64();
 #endif
-        cs.seen_m3 = cs.seen_m2 = cs.seen_m1 = cs.seen_p1 = cs.seen_p2 = cs.seen_p3 = A.tag_base;
+        cs.seen_sh = seen_sh;
+        cs.tcol = tile + slot_base * pitch + tid;
+        cs.slot_words = (long long)st_tile_rows(T) * pitch;
+        cs.box0 = A.mail + (long long)cta * ST_RING * cs.slot_words + (long long)slot_base * pitch + tid;
+        cs.dest_step = st_dest_step(A);
         Waiter wt(A, abort_flag);
         bool stopped_early = false;
         const int h_lo = tab[0].hold_lo, h_hi = tab[0].hold_hi;      // rows held at the top of EVERY sweep
@@ -889,7 +891,7 @@ static void set_why(char *why, size_t n, const char *fmt, ...)
     va_end(ap);
 }
 
-static size_t strips_fixed_smem() { return ST_NSTG * 8 + ST_MAX_SIDES * ST_MAX_SIDE * sizeof(MacroEntry) + 16 + (ST_MAX_WARPS + 2) * 8; }
+static size_t strips_fixed_smem() { return ST_NSTG * 8 + ST_MAX_SIDES * ST_MAX_SIDE * sizeof(MacroEntry) + 16 + (ST_MAX_WARPS + 2) * 8 + 32; }
 
 // Brute-force check of one strip height against every geometry of a sweep (host only, closed forms).
 static bool strips_check_T(int H, int NS, int T, const int *sides, int n_sides, int *max_rows, int *max_hop,
