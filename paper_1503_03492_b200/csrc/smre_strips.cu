@@ -417,9 +417,10 @@ __device__ __forceinline__ void macro_steps(const StripArgs &A, const MacroEntry
                                             int j, int cta, ComputeState &cs, int warp, int lane, int NTL, bool handoff,
                                             Waiter &w)
 {
+    (void)j; (void)cta; (void)handoff; (void)w;
     constexpr int CW = (32 / S) * S;
     const int pitch = PITCH ? PITCH : A.Wq;
-    const int W = A.W, NR = A.NR;
+    int W = A.W, NR = A.NR;
     const int src = (lane / S) * S;
     const float cth = e.c, sq = e.sqrt_c;
     const int rows = e.rows, nb = e.nb;
@@ -432,9 +433,13 @@ __device__ __forceinline__ void macro_steps(const StripArgs &A, const MacroEntry
     int w_end = lane < CW ? warp * CW + src + S : (1 << 28);   // end of the lane's window at ox = 0
     float *xt = tile + e.xoff + col0;
     float *qg = A.q + e.qoff + col0;
-    const size_t q_step = (size_t)A.Btot * A.H * pitch + 1;    // next family's plane, next column
+    size_t q_step = (size_t)A.Btot * A.H * pitch + 1;          // next family's plane, next column
+    asm volatile("" : "+l"(q_step));                            // kept in registers: rebuilt from the kernel parameters
+    asm volatile("" : "+r"(NTL));                               // it sat on the path to the step barrier
     const float *qcol = ring + col0;
-    const bool elim = A.elim != 0;
+    int elim_i = A.elim;
+    asm volatile("" : "+r"(W), "+r"(NR), "+r"(elim_i));
+    const bool elim = elim_i != 0;
 #pragma unroll 1
     for (int ox = 0; ox < S; ++ox) {
         const bool on = w_end <= W;                            // the window lies inside the image (reading A6)
@@ -1012,9 +1017,9 @@ StripPlan *strips_plan_create(int H, int W, int B, int Wq, const int *sides, con
     p->F = F;
     p->threads = (p->NWC + 2) * 32;                               // compute warps + waiter + issuer
     // two builds: up to 18 warps with 96 registers, else 64 (measured on C1, 21 warps: 64 and 88 registers run alike)
-    const bool big = p->threads > 576;
-    if (Wq == 512) p->kernel = big ? kernel_ptr<512, 1024>() : kernel_ptr<512, 576>();
-    else p->kernel = big ? kernel_ptr<0, 1024>() : kernel_ptr<0, 576>();
+    const bool big = p->threads > 672;
+    if (Wq == 512) p->kernel = big ? kernel_ptr<512, 1024>() : kernel_ptr<512, 672>();
+    else p->kernel = big ? kernel_ptr<0, 1024>() : kernel_ptr<0, 672>();
     p->smem_bytes = (size_t)st_tile_rows(p->T) * Wq * 4 + (size_t)p->NR * Wq * 4 + strips_fixed_smem();
     if (const char *e = getenv("SMRE_DENSE_STORES")) p->elim = atoi(e) ? 0 : 1;
     if (const char *e = getenv("SMRE_TIMEOUT_MS")) {
