@@ -133,6 +133,18 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 // protocol bug or a lost CTA ends the kernel with an error code instead of hanging the GPU.
 enum { ST_W_QFULL = 1, ST_W_ALLOW = 3, ST_W_MAIL = 4, ST_W_SWEEP = 5, ST_W_DONE = 6 };
 
+// the rare part of a wait (every 64th failed poll): returns the new start time, or ~0 to give up
+__device__ __noinline__ unsigned long long st_wait_check(const StripArgs &A, unsigned *abort_flag, unsigned long long t0, int what)
+{
+    const unsigned long long now = globaltimer_ns();
+    if (t0 == 0) return now;
+    if (ld_relaxed_gpu32(A.status) != 0 || now - t0 > A.timeout_ns) {
+        atomicCAS(A.status, 0u, (unsigned)what | ((unsigned)blockIdx.x << 8));
+        *(volatile unsigned *)abort_flag = 1u;
+        return ~0ull;
+    }
+    return t0;
+}
 struct Waiter {
     const StripArgs &A;
     unsigned *abort_flag;                    // shared memory
@@ -141,18 +153,12 @@ struct Waiter {
     __device__ Waiter(const StripArgs &a, unsigned *f) : A(a), abort_flag(f) {}
     __device__ __forceinline__ void begin() { spins = 0; t0 = 0; }
     // call after a failed poll; true -> give up
-    __device__ __noinline__ bool slow(int what)
+    __device__ __forceinline__ bool slow(int what)
     {
         if (*(volatile unsigned *)abort_flag) return true;
         if ((++spins & 63u) != 0) return false;
-        const unsigned long long now = globaltimer_ns();
-        if (t0 == 0) { t0 = now; return false; }
-        if (ld_relaxed_gpu32(A.status) != 0 || now - t0 > A.timeout_ns) {
-            atomicCAS(A.status, 0u, (unsigned)what | ((unsigned)blockIdx.x << 8));
-            *(volatile unsigned *)abort_flag = 1u;
-            return true;
-        }
-        return false;
+        t0 = st_wait_check(A, abort_flag, t0, what);
+        return t0 == ~0ull;
     }
 };
 
@@ -170,12 +176,13 @@ struct __align__(16) MacroEntry {
     // d = -HOPS..-1, +1..+HOPS (k = 0..2*HOPS-1); rows [recv_lo[i], recv_hi[i]) arrive (above / below what is kept)
     short send_lo[2 * ST_HOPS], send_hi[2 * ST_HOPS];
     short recv_lo[2], recv_hi[2];
-    short ae_last, pad;                 // end of the last whole window of the macro step's LAST family (ox = s - 1)
-    // where each active row goes at the hand-off, 4 bits per row from `lo` on: 0 stays, 1..6 = strip j-3..j-1, j+1..j+3
-    unsigned long long sendmap;
-    long long pad2;
+    int pad0;
+    long long pad1;
+    // the same hand-off in one 16-byte load, in TILE rows (image row - j T + T / 2, 0 .. T + 7): 10 bits per run,
+    // first row in bits 0-3, number of rows in bits 4-9; splan: the six send runs (k = 0..5), rplan: the two arrival runs
+    unsigned long long splan, rplan;
 };
-static_assert(sizeof(MacroEntry) == 96, "MacroEntry");
+static_assert(sizeof(MacroEntry) == 96 && offsetof(MacroEntry, splan) % 16 == 0, "MacroEntry");
 
 // ------------------------------------------------------------------------------------------------ window sums
 // Sum over the S lanes of a window, delivered to every lane of it.  col = the lane's column sum; src = lane of the
@@ -282,20 +289,16 @@ struct ComputeState {
 #endif
     int pos = 0;                        // q ring: next free row
     unsigned mc = 0;                    // transitions done
-    float *tcol;                        // my column of the tile, addressed by image row: tcol[y * pitch]
+    float *tcol;                        // my column of the tile: tcol[t * pitch], t = tile row
     unsigned long long *box0;           // my column of slot 0 of my mailbox, addressed the same way
     long long slot_words, dest_step;    // next slot of my mailbox; same slot of the next strip's mailbox
     unsigned *seen_sh;                  // shared memory [6]: cached progress words of strips j-3..j-1, j+1..j+3
                                         // (flow control of their mailbox rings)
 };
 
-// Mailbox slot of transition number mc in the mailbox of the strip of CTA `cta`, addressed by image row / column:
-// word of (row y, column c) = base[y * Wq + c]; the same slot of strip j + d lies d * st_dest_step() further on.
-__device__ __forceinline__ unsigned long long *st_mailbox(const StripArgs &A, int cta, int j, unsigned mc)
-{
-    const long long slot_words = (long long)st_tile_rows(A.T) * A.Wq;
-    return A.mail + ((long long)cta * ST_RING + mc % ST_RING) * slot_words + (long long)(A.T / 2 - j * A.T) * A.Wq;
-}
+// Mailboxes: CTA `cta` owns ST_RING slots of st_tile_rows(T) rows of Wq words; transition number mc uses slot
+// mc % ST_RING; a row is filed under the RECEIVER's tile row.  The same slot of strip j + d lies d * st_dest_step()
+// further on (next mailbox, tile rows shifted by T).
 __device__ __forceinline__ long long st_dest_step(const StripArgs &A)
 {
     return (long long)ST_RING * st_tile_rows(A.T) * A.Wq - (long long)A.T * A.Wq;
@@ -321,13 +324,12 @@ __device__ __forceinline__ void st_ring_space(const StripArgs &A, int cta, int d
 // bottom) and the columns outside its windows (left / right remainder).  Sends wait for nothing but ring space, so
 // the hand-offs of one transition cannot form a cycle.  A thread owns column tid (W <= compute threads).
 // A row travels to slot (receiver's tile row) of the receiver's mailbox, whoever sends it.
-__device__ __forceinline__ void transition(const StripArgs &A, float *tile, int pitch, int j, int cta,
-                                           const MacroEntry &e, ComputeState &cs, int tid, int NT, Waiter &w)
+__device__ __forceinline__ void transition(const StripArgs &A, int pitch, int j, int cta, unsigned long long splan,
+                                           unsigned long long rplan, ComputeState &cs, int tid, int NT, Waiter &w)
 {
     constexpr int MAXR = 8;                                    // rows requested at once
     static_assert(ST_HOPS == 3, "the sends below are written out for three hops");
     static_assert((ST_RING & (ST_RING - 1)) == 0, "ST_RING must be a power of two");
-    const int NS = A.NS;
     const unsigned mc = ++cs.mc;
     const unsigned tag = A.tag_base + mc;
     if (ST_KO(A, 1)) { bar_sync(2, NT); return; }
@@ -336,26 +338,26 @@ __device__ __forceinline__ void transition(const StripArgs &A, float *tile, int 
     cs.t_macro += c0 - cs.t_last;
 #endif
     const bool mine = tid < A.W;
-    float *const tcol = cs.tcol;                                // tcol[y * pitch]: image row y, my column
-    unsigned long long *const box = cs.box0 + (size_t)(mc & (ST_RING - 1)) * cs.slot_words;   // box[y * pitch]
-    const long long dest_step = cs.dest_step;
+    float *const trow = cs.tcol;                                // trow[t * pitch]: tile row t, my column
+    unsigned long long *const box = cs.box0 + (size_t)(mc & (ST_RING - 1)) * cs.slot_words;   // box[t * pitch]
 
-    // departures first: they are what the strips around are waiting for
-    auto send = [&](int d, int lo, int hi, int k) {
-        if (lo >= hi) return;
-        unsigned seen = *(volatile unsigned *)(cs.seen_sh + k);
-        st_ring_space(A, cta, d, tag, mc, seen, w);
-        if (!mine) return;
-        unsigned long long *dst = box + d * dest_step;
-        for (int y = lo; y < hi; ++y)
-            st_relaxed_gpu64(dst + y * pitch, pack_word(tag, tcol[y * pitch]));
-    };
-    send(-1, e.send_lo[2], e.send_hi[2], 2);
-    send(+1, e.send_lo[3], e.send_hi[3], 3);
-    send(-2, e.send_lo[1], e.send_hi[1], 1);
-    send(+2, e.send_lo[4], e.send_hi[4], 4);
-    send(-3, e.send_lo[0], e.send_hi[0], 0);
-    send(+3, e.send_lo[5], e.send_hi[5], 5);
+    // departures first: they are what the strips around are waiting for.  The plan is one 64-bit word, so the six
+    // runs cost a few ALU instructions each and no dependent shared-memory loads.
+    if (splan != 0ull) {
+#pragma unroll
+        for (int k = 0; k < 2 * ST_HOPS; ++k) {
+            const unsigned f = (unsigned)(splan >> (10 * k)) & 1023u;
+            if (f == 0u) continue;
+            const int d = k < ST_HOPS ? k - ST_HOPS : k - ST_HOPS + 1;
+            unsigned seen = *(volatile unsigned *)(cs.seen_sh + k);
+            st_ring_space(A, cta, d, tag, mc, seen, w);
+            if (!mine) continue;
+            const int lo = (int)(f & 15u), n = (int)(f >> 4);
+            unsigned long long *dst = box + d * cs.dest_step + lo * pitch;
+            const float *src = trow + lo * pitch;
+            for (int r = 0; r < n; ++r) st_relaxed_gpu64(dst + r * pitch, pack_word(tag, src[r * pitch]));
+        }
+    }
 #ifdef SMRE_ST_KO
     const long long c1 = clock64();
 #endif
@@ -363,14 +365,13 @@ __device__ __forceinline__ void transition(const StripArgs &A, float *tile, int 
     // neighbour asks now and files the answer in shared memory after the arrivals
     unsigned s_new = 0;
     const int nd = tid < ST_HOPS ? tid - ST_HOPS : tid - ST_HOPS + 1;       // tid 0..5 -> strip j-3..j-1, j+1..j+3
-    const bool asks = tid < 2 * ST_HOPS && j + nd >= 0 && j + nd < NS;
+    const bool asks = tid < 2 * ST_HOPS && j + nd >= 0 && j + nd < A.NS;
     if (asks) s_new = ld_relaxed_gpu32(A.done + (size_t)(cta + nd) * 32);
 
-    // arrivals: all words of a batch are requested at once; a word whose tag is right goes to the tile, the others
-    // are requested again.  The loop is kept short on purpose: with every compute warp in it, the time of one round
-    // is set by the instructions it issues, and an arrival is seen one round late on average.
-    const int n0 = e.recv_hi[0] - e.recv_lo[0], n = n0 + e.recv_hi[1] - e.recv_lo[1];
-    if (mine && n > 0) {
+    // arrivals: up to two runs of consecutive tile rows.  All words of a batch are requested at once; a word whose
+    // tag is right goes to the tile, the others are requested again.
+    if (mine && rplan != 0ull) {
+        const int lo0 = (int)(rplan & 15u), n0 = (int)(rplan >> 4) & 63, lo1 = (int)(rplan >> 10) & 15, n = n0 + ((int)(rplan >> 14) & 63);
         w.begin();
         for (int r0 = 0; r0 < n; r0 += MAXR) {
             int off[MAXR];
@@ -378,7 +379,7 @@ __device__ __forceinline__ void transition(const StripArgs &A, float *tile, int 
 #pragma unroll
             for (int r = 0; r < MAXR; ++r) {
                 const int i = r0 + r;
-                off[r] = (i < n0 ? e.recv_lo[0] + i : e.recv_lo[1] + (i - n0)) * pitch;
+                off[r] = (i < n0 ? lo0 + i : lo1 + (i - n0)) * pitch;
                 if (i < n) missing |= 1u << r;
             }
             for (;;) {
@@ -389,7 +390,7 @@ __device__ __forceinline__ void transition(const StripArgs &A, float *tile, int 
 #pragma unroll
                 for (int r = 0; r < MAXR; ++r)
                     if ((missing >> r & 1u) && (unsigned)(wd[r] >> 32) == tag) {
-                        tcol[off[r]] = __uint_as_float((unsigned)wd[r]);
+                        trow[off[r]] = __uint_as_float((unsigned)wd[r]);
                         missing &= ~(1u << r);
                     }
                 if (ST_KO(A, 64)) missing = 0;
@@ -735,14 +736,15 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
         // what I hold next and do not hold now: above / below what I keep
         e.recv_lo[0] = (short)nlo; e.recv_hi[0] = (short)max(nlo, min(nhi, olo));
         e.recv_lo[1] = (short)min(nhi, max(nlo, ohi)); e.recv_hi[1] = (short)nhi;
-        e.ae_last = (short)((s - 1) + ((W - (s - 1)) / s) * s);
-        e.pad = 0; e.pad2 = 0;
-        e.sendmap = 0;
-        for (int i = 0; i < hi - lo && i < 16; ++i) {            // where the active row lo + i goes
-            const int y = lo + i;
-            for (int k = 0; k < 2 * ST_HOPS; ++k)
-                if (y >= e.send_lo[k] && y < e.send_hi[k]) e.sendmap |= (unsigned long long)(k + 1) << (4 * i);
-        }
+        e.pad0 = 0; e.pad1 = 0;
+        const int tb = T / 2 - j * T;                            // image row -> tile row
+        e.splan = 0; e.rplan = 0;
+        for (int k = 0; k < 2 * ST_HOPS; ++k)
+            if (e.send_hi[k] > e.send_lo[k])
+                e.splan |= (unsigned long long)((e.send_lo[k] + tb) | ((e.send_hi[k] - e.send_lo[k]) << 4)) << (10 * k);
+        for (int i = 0; i < 2; ++i)
+            if (e.recv_hi[i] > e.recv_lo[i])
+                e.rplan |= (unsigned long long)((e.recv_lo[i] + tb) | ((e.recv_hi[i] - e.recv_lo[i]) << 4)) << (10 * i);
         tab[threadIdx.x] = e;
     }
     if (threadIdx.x == 0) {
@@ -774,9 +776,9 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
         cs.t_last = clock64();
 #endif
         cs.seen_sh = seen_sh;
-        cs.tcol = tile + slot_base * pitch + tid;
+        cs.tcol = tile + tid;
         cs.slot_words = (long long)st_tile_rows(T) * pitch;
-        cs.box0 = A.mail + (long long)cta * ST_RING * cs.slot_words + (long long)slot_base * pitch + tid;
+        cs.box0 = A.mail + (long long)cta * ST_RING * cs.slot_words + tid;
         cs.dest_step = st_dest_step(A);
         Waiter wt(A, abort_flag);
         bool stopped_early = false;
@@ -830,6 +832,7 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
             }
             for (int m = 0; m < M; ++m) {
                 const MacroEntry e = tab[m];
+                const unsigned long long splan = e.splan, rplan = e.rplan;
                 const bool staged = sweep > 0 && !ST_KO(A, 2);
                 const bool handoff = !(m + 1 == M && sweep + 1 == A.n_sweeps);   // none after the very last one
 #define SMRE_RUN(S_)                                                                                                   \
@@ -839,7 +842,7 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
                 }
 #undef SMRE_RUN
                 if (!handoff) break;
-                transition(A, tile, pitch, j, cta, e, cs, tid, NT, wt);
+                transition(A, pitch, j, cta, splan, rplan, cs, tid, NT, wt);
             }
         }
         if (A.tol_mode && !stopped_early && j == 0 && tid == 0 && A.sweeps_done) A.sweeps_done[frame] = A.n_sweeps;
