@@ -652,8 +652,10 @@ __device__ void issuer_warp(const StripArgs &A, const MacroEntry *tab, int M, fl
         }
         if (have < need) {
             wt.begin();
-            while ((have = ld_acquire_cta(progress)) < need)
+            while ((have = ld_acquire_cta(progress)) < need) {
+                __nanosleep(200);                               // far ahead of the compute warps: do not take their issue slots
                 if (wt.slow(ST_W_QFULL)) break;
+            }
         }
         fence_proxy_async();                                    // generic-proxy q stores -> async-proxy reads
         if (lane < k) mbar_arrive_expect_tx(&full[(head.n + lane) % ST_NSTG], (uint32_t)rows * row_bytes);
