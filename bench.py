@@ -40,12 +40,12 @@ def measured_peaks():
 
 
 def profile_metric(workload_name, key):
-    """A per-launch number taken from the committed ncu summaries (profiles/r02_measured.json, written from the
+    """A per-launch number taken from the committed ncu summaries (profiles/r02_measured.txt, written from the
     captures named there): DRAM traffic of the C1 kernel, thread-instructions of the ICD kernels.  None if absent."""
-    p = os.path.join(ROOT, "profiles", "r02_measured.json")
+    p = os.path.join(ROOT, "profiles", "r02_measured.txt")
     try:
         d = json.load(open(p))
-        return d.get(workload_name, {}).get(key), "profiles/r02_measured.json (" + d.get("_source", "?") + ")"
+        return d.get(workload_name, {}).get(key), "profiles/r02_measured.txt (" + d.get("_source", "?") + ")"
     except (OSError, ValueError):
         return None, None
 
