@@ -24,7 +24,9 @@
  * symmetries, ICD == composition of restricted standard runs == explicit
  * tile-by-tile solve, counts, the all-windows checker against a strided-view
  * sum, the stop rules of the tolerance modes against fixed-count runs and an
- * independent tile-wise solve.  No function here is "parity unpinned".
+ * independent tile-wise solve; the PSF operator against scipy and the 2-D
+ * definition, the ADMM against the problem it solves (projection limit, KKT
+ * system, SLSQP).  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdlib.h>
@@ -536,4 +538,137 @@ int smre_oracle_cumulant2(const double *stack, int n, int H, int W, double *c2_o
         c2_out[i] = m2 - m1 * m1;
     }
     return 0;
+}
+
+/* ===========================================================================
+ * The ADMM around the projection (Alg. 1, Eq. 9-13; parameters App. B,
+ * PAPER.md:697-753).  DESIGN.md readings A-ADMM-1..9.
+ *
+ * Problem (Eq. 10):   min  G(eps) + R(z)   s.t.  I = A * x + eps,  z = x,
+ * G = indicator of the multi-resolution constraint set (Eq. 5), R(z) = (lambda / 2) ||z||^2 ("we use the generic L2
+ * norm as regularization"; lambda = `regularization` of App. B).
+ *
+ * A ("approximated as Gaussian kernel with the standard deviation sigma_PSF"): separable, taps
+ * g[t] = exp(-t^2 / (2 sigma^2)), |t| <= radius = ceil(3 sigma), normalised to sum 1; the image is continued by
+ * zero outside (A-ADMM-2), so A is a symmetric matrix and A^T * = A *.  sigma = 0: A = identity.
+ * ------------------------------------------------------------------------- */
+int smre_oracle_gauss_taps(double sigma, double *taps, int max_taps)
+{
+    if (sigma < 0.0 || !taps) return -1;
+    int radius = (int)ceil(3.0 * sigma);
+    if (2 * radius + 1 > max_taps) return -1;
+    double sum = 0.0;
+    for (int t = -radius; t <= radius; ++t) {
+        taps[t + radius] = sigma > 0.0 ? exp(-(double)t * t / (2.0 * sigma * sigma)) : 1.0;
+        sum += taps[t + radius];
+    }
+    for (int t = 0; t <= 2 * radius; ++t) taps[t] /= sum;
+    return radius;
+}
+
+/* out = A * x: rows first, then columns (two plain passes, zero outside the image). */
+int smre_oracle_gauss_conv(const double *x, int H, int W, double sigma, double *out)
+{
+    double taps[257];
+    int radius = smre_oracle_gauss_taps(sigma, taps, 257);
+    if (radius < 0 || !x || !out || H <= 0 || W <= 0) return -1;
+    double *tmp = (double *)malloc((size_t)H * W * sizeof(double));
+    if (!tmp) return -2;
+    for (int y = 0; y < H; ++y)
+        for (int c = 0; c < W; ++c) {
+            double a = 0.0;
+            for (int t = -radius; t <= radius; ++t) {
+                int cc = c + t;
+                if (cc >= 0 && cc < W) a += taps[t + radius] * x[(size_t)y * W + cc];
+            }
+            tmp[(size_t)y * W + c] = a;
+        }
+    for (int y = 0; y < H; ++y)
+        for (int c = 0; c < W; ++c) {
+            double a = 0.0;
+            for (int t = -radius; t <= radius; ++t) {
+                int yy = y + t;
+                if (yy >= 0 && yy < H) a += taps[t + radius] * tmp[(size_t)yy * W + c];
+            }
+            out[(size_t)y * W + c] = a;
+        }
+    free(tmp);
+    return 0;
+}
+
+/* Alg. 1 with the z = x splitting of Eq. 10, in the order of the algorithm box:
+ *
+ *   x_{r+1}   = x_r - (1 / (2 gamma)) grad_x L(x_r)                                  (Eq. 11, reading A-ADMM-3)
+ *               grad_x L = -A^T * (rho1 (I - A * x_r - eps_r) + Y1) + rho2 (x_r - z_r) + Y2
+ *   eps_{r+1} = P_G(I - A * x_{r+1} + Y1 / rho1)                                     (Eq. 12; Dykstra, variant 0 / 1,
+ *                                                                                     n_sweeps from q = 0, A13)
+ *   z_{r+1}   = (rho2 x_{r+1} + Y2) / (lambda + rho2)                                (argmin_z of L; A-ADMM-4)
+ *   Y1       += alpha1 (I - A * x_{r+1} - eps_{r+1})                                  (Alg. 1, steepest ascent)
+ *   Y2       += alpha2 (x_{r+1} - z_{r+1})
+ *
+ * from x_0 = z_0 = 0, eps_0 = 0, Y = 0 (A-ADMM-5: with x_0 = I the first x-update is the identity and the `while`
+ * would end at once), while r < max_iter and
+ * ( ||x_r - x_{r-1}||_2 > delta  or  ||I - (A * x_r + eps_r)||_2 > delta ): the loop ends when BOTH are small
+ * (A-ADMM-6: Alg. 1 prints `and`, which would end the loop in the first iteration whose projection absorbs the
+ * residual completely -- the residual is exactly 0 whenever the argument of P_G is feasible -- long before x has
+ * settled; App. B states "Finish when |x_r - x_{r-1}| < tolerance").
+ *
+ * Outputs: x, eps, z, Y1, Y2 [H*W] (any may be null), *iters = iterations done, hist[2 * max_iter] (may be null) =
+ * the two norms after each iteration.
+ */
+int smre_oracle_admm(const double *I, int H, int W, const int *sides, const double *c, int n_sides, int variant,
+                     int n_sweeps, double sigma, double rho1, double rho2, double alpha1, double alpha2,
+                     double lambda, double gamma, double delta, int max_iter,
+                     double *x_out, double *eps_out, double *z_out, double *y1_out, double *y2_out,
+                     int *iters, double *hist)
+{
+    if (!I || H <= 0 || W <= 0 || !sides || !c || n_sides <= 0 || n_sweeps <= 0 || max_iter <= 0) return -1;
+    if (!(rho1 > 0.0) || !(rho2 > 0.0) || !(gamma > 0.0) || lambda < 0.0 || sigma < 0.0) return -1;
+    size_t N = (size_t)H * W;
+    double *buf = (double *)calloc(9 * N, sizeof(double));
+    if (!buf) return -2;
+    double *x = buf, *eps = buf + N, *z = buf + 2 * N, *Y1 = buf + 3 * N, *Y2 = buf + 4 * N;
+    double *Ax = buf + 5 * N, *w = buf + 6 * N, *Aw = buf + 7 * N, *X = buf + 8 * N;
+    int rc = 0, r = 0;
+    while (r < max_iter) {
+        /* x-update */
+        if ((rc = smre_oracle_gauss_conv(x, H, W, sigma, Ax)) != 0) break;
+        for (size_t i = 0; i < N; ++i) w[i] = rho1 * (I[i] - Ax[i] - eps[i]) + Y1[i];
+        if ((rc = smre_oracle_gauss_conv(w, H, W, sigma, Aw)) != 0) break;          /* A^T * = A * */
+        double dx2 = 0.0;
+        for (size_t i = 0; i < N; ++i) {
+            double g = -Aw[i] + rho2 * (x[i] - z[i]) + Y2[i];
+            double xn = x[i] - g / (2.0 * gamma);
+            dx2 += (xn - x[i]) * (xn - x[i]);
+            x[i] = xn;
+        }
+        /* eps-update: the projection */
+        if ((rc = smre_oracle_gauss_conv(x, H, W, sigma, Ax)) != 0) break;
+        for (size_t i = 0; i < N; ++i) X[i] = I[i] - Ax[i] + Y1[i] / rho1;
+        if (variant == 0) rc = smre_oracle_std(X, H, W, sides, c, n_sides, n_sweeps, eps, NULL, NULL);
+        else rc = smre_oracle_icd(X, H, W, sides, c, n_sides, n_sweeps, eps);
+        if (rc != 0) break;
+        /* z-update, dual ascent */
+        double res2 = 0.0;
+        for (size_t i = 0; i < N; ++i) {
+            z[i] = (rho2 * x[i] + Y2[i]) / (lambda + rho2);
+            double r1 = I[i] - Ax[i] - eps[i];
+            Y1[i] += alpha1 * r1;
+            Y2[i] += alpha2 * (x[i] - z[i]);
+            res2 += r1 * r1;
+        }
+        ++r;
+        if (hist) { hist[2 * (r - 1)] = sqrt(dx2); hist[2 * (r - 1) + 1] = sqrt(res2); }
+        if (!(sqrt(dx2) > delta || sqrt(res2) > delta)) break;
+    }
+    if (rc == 0) {
+        if (x_out) memcpy(x_out, x, N * sizeof(double));
+        if (eps_out) memcpy(eps_out, eps, N * sizeof(double));
+        if (z_out) memcpy(z_out, z, N * sizeof(double));
+        if (y1_out) memcpy(y1_out, Y1, N * sizeof(double));
+        if (y2_out) memcpy(y2_out, Y2, N * sizeof(double));
+        if (iters) *iters = r;
+    }
+    free(buf);
+    return rc;
 }

@@ -84,6 +84,14 @@ def _load():
         lib.smre_oracle_cumulant2.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
         lib.smre_oracle_window_sums.restype = ctypes.c_int
         lib.smre_oracle_window_sums.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp]
+        lib.smre_oracle_gauss_conv.restype = ctypes.c_int
+        lib.smre_oracle_gauss_conv.argtypes = [_dp, ctypes.c_int, ctypes.c_int, ctypes.c_double, _dp]
+        lib.smre_oracle_gauss_taps.restype = ctypes.c_int
+        lib.smre_oracle_gauss_taps.argtypes = [ctypes.c_double, _dp, ctypes.c_int]
+        lib.smre_oracle_admm.restype = ctypes.c_int
+        lib.smre_oracle_admm.argtypes = [
+            _dp, ctypes.c_int, ctypes.c_int, _ip, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int] + [ctypes.c_double] * 8 + [
+            ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _ip, _dp]
         _lib = lib
     return _lib
 
@@ -304,6 +312,46 @@ def cumulant2(stack):
     out = np.empty((H, W), np.float64)
     _check(lib.smre_oracle_cumulant2(_p(stack, _dp), n, H, W, _p(out, _dp)), "smre_oracle_cumulant2")
     return out
+
+
+def gauss_taps(sigma):
+    """Normalised taps of the Gaussian PSF, radius ceil(3 sigma) (reading A-ADMM-2)."""
+    lib = _load()
+    t = np.zeros(257, np.float64)
+    r = lib.smre_oracle_gauss_taps(float(sigma), _p(t, _dp), 257)
+    if r < 0:
+        raise RuntimeError("smre_oracle_gauss_taps failed")
+    return t[:2 * r + 1].copy()
+
+
+def gauss_conv(x, sigma):
+    """A * x: separable Gaussian of standard deviation sigma, zero outside the image (= A^T * x)."""
+    lib = _load()
+    x = _f64(x)
+    H, W = x.shape
+    out = np.empty((H, W), np.float64)
+    _check(lib.smre_oracle_gauss_conv(_p(x, _dp), H, W, float(sigma), _p(out, _dp)), "smre_oracle_gauss_conv")
+    return out
+
+
+def admm(I, sides, c, variant, n_sweeps, sigma, rho1, rho2, alpha1, alpha2, lam, gamma, delta, max_iter):
+    """Alg. 1 with the z = x splitting (smre_oracle.c has the update rules and the readings).
+    Returns a dict: x, eps, z, Y1, Y2, iters, hist[iters, 2] = (||x_r - x_{r-1}||, ||I - A x_r - eps_r||)."""
+    lib = _load()
+    I = _f64(I)
+    H, W = I.shape
+    sides = _i32(sides)
+    c = _f64(c)
+    outs = [np.empty((H, W), np.float64) for _ in range(5)]
+    it = np.zeros(1, np.int32)
+    hist = np.zeros(2 * int(max_iter), np.float64)
+    v = 0 if variant in ("standard", 0) else 1
+    _check(lib.smre_oracle_admm(_p(I, _dp), H, W, _p(sides, _ip), _p(c, _dp), len(sides), v, int(n_sweeps),
+                                float(sigma), float(rho1), float(rho2), float(alpha1), float(alpha2), float(lam),
+                                float(gamma), float(delta), int(max_iter), *[_p(o, _dp) for o in outs],
+                                _p(it, _ip), _p(hist, _dp)), "smre_oracle_admm")
+    n = int(it[0])
+    return dict(x=outs[0], eps=outs[1], z=outs[2], Y1=outs[3], Y2=outs[4], iters=n, hist=hist[:2 * n].reshape(n, 2))
 
 
 def project(y, sides, c, n_sweeps, variant):
