@@ -213,6 +213,47 @@ smre_status smre_calibrate(int H, int W, int n_frames, const int *sides, int n_s
  */
 smre_status smre_cumulant2(int H, int W, int n_frames, const float *stack_dev, float *c2_out_dev, void *cuda_stream);
 
+/* Shape the handle was created for (any pointer may be NULL). */
+smre_status smre_shape(smre_handle h, int *H, int *W, int *batch);
+
+/* ---- The ADMM around the projection (Alg. 1, Eq. 9-13) -----------------
+ * Solves Eq. 10,  min G(eps) + (lambda/2) ||z||^2  s.t.  I = A * x + eps,  z = x,  with G the multi-resolution
+ * constraint of the handle (its sides and thresholds) and A a Gaussian PSF of standard deviation sigma_psf
+ * (taps exp(-t^2 / 2 sigma^2), |t| <= ceil(3 sigma) <= 32, normalised, zero outside the image; 0 = identity).
+ * One iteration, in Alg. 1's order (the readings A-ADMM-1..9 of DESIGN.md state what the paper leaves open):
+ *     x   <- x - grad_x L / (2 gamma),  grad_x L = -A^T * (rho1 (I - A * x - eps) + Y1) + rho2 (x - z) + Y2   (Eq. 11)
+ *     eps <- P_G(I - A * x + Y1 / rho1)          (Eq. 12: smre_project on `h`, n_sweeps sweeps / cycles from q = 0)
+ *     z   <- (rho2 x + Y2) / (lambda + rho2)
+ *     Y1  += alpha1 (I - A * x - eps),  Y2 += alpha2 (x - z)
+ * from x = z = eps = Y = 0, until ||x_r - x_{r-1}||_2 <= delta and ||I - A * x_r - eps_r||_2 <= delta, at most
+ * max_iter iterations.  All arithmetic is fp32 on the device (the two norms are summed in fp64 in a fixed order, so
+ * a run is repeatable bit for bit); the host only enqueues and reads the stop flag every `check_every` iterations
+ * (<= 0: 8); kernels enqueued behind the stop do nothing, so the result is that of the iteration that stopped.
+ * App. B of the paper: rho1 = 6.192, rho2 = 1.8, alpha1 = 1.2, alpha2 = 0.12, lambda = 1, delta = 1e-3; gamma is
+ * not given there: the x step is stable for 2 gamma >= rho1 + rho2.
+ *   h             handle with batch 1 and the shape H x W (either variant; its schedule is used as set)
+ *   I_dev         [H][W] device, read only;  x_out_dev [H][W] device: the estimate x;  eps_out_dev: the residual, or NULL
+ *   iters_out     HOST int, or NULL: iterations done
+ *   hist_out_dev  device [2 * max_iter] or NULL: the two norms after every iteration
+ * Synchronous (returns after the stream has drained).  Allocates and frees its workspace (10 images) per call.
+ * Errors: SMRE_EINVAL (pointers, shape mismatch, batch != 1, parameters out of range), SMRE_EUNSUPPORTED
+ * (sigma_psf > 10.6), SMRE_ENOMEM, SMRE_ECUDA, and whatever smre_project returns. */
+typedef struct {
+    float sigma_psf;
+    float rho1, rho2, alpha1, alpha2, lambda, gamma;
+    float delta;
+    int max_iter;
+    int n_sweeps;
+    int check_every;
+} smre_admm_params;
+smre_status smre_admm(smre_handle h, int H, int W, const float *I_dev, const smre_admm_params *p, float *x_out_dev,
+                      float *eps_out_dev, int *iters_out, float *hist_out_dev, void *cuda_stream);
+
+/* out = A * in with the PSF operator of smre_admm (rows into tmp_dev, columns into out_dev; all [H][W] device,
+ * in_dev may not alias the others).  Asynchronous on cuda_stream. */
+smre_status smre_psf_apply(int H, int W, float sigma_psf, const float *in_dev, float *tmp_dev, float *out_dev,
+                           void *cuda_stream);
+
 /* Text of the last error on the calling thread ("" if none).  Never NULL. */
 const char *smre_last_error(void);
 

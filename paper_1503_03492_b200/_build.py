@@ -7,7 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libsmre.so")
-SOURCES = ["smre_api.cu", "smre_family.cu", "smre_icd.cu", "smre_conveyor.cu", "smre_conveyor_plan.cu", "smre_strips.cu", "smre_noalloc.cu", "smre_calibrate.cu"]
+SOURCES = ["smre_api.cu", "smre_family.cu", "smre_icd.cu", "smre_conveyor.cu", "smre_conveyor_plan.cu", "smre_strips.cu", "smre_noalloc.cu", "smre_calibrate.cu", "smre_admm.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared",

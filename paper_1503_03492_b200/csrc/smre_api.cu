@@ -365,6 +365,15 @@ extern "C" smre_status smre_project_host(smre_handle h, const float *y_host, flo
     return SMRE_OK;
 }
 
+extern "C" smre_status smre_shape(smre_handle h, int *H, int *W, int *batch)
+{
+    if (!h) { set_last_error("smre_shape: null handle"); return SMRE_EINVAL; }
+    if (H) *H = h->H;
+    if (W) *W = h->W;
+    if (batch) *batch = h->B;
+    return SMRE_OK;
+}
+
 extern "C" smre_status smre_info(smre_handle h, int *n_families, long long *windows_per_sweep,
                                  long long *increment_bytes)
 {

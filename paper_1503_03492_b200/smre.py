@@ -18,10 +18,19 @@ SMRE_SCHED_AUTO, SMRE_SCHED_GRAPH, SMRE_SCHED_PERSISTENT, SMRE_SCHED_STRIPS = 0,
 _STATUS = {0: "SMRE_OK", 1: "SMRE_EINVAL", 2: "SMRE_EUNSUPPORTED", 3: "SMRE_ENOMEM", 4: "SMRE_ECUDA"}
 
 # every symbol include/smre.h declares
+class AdmmParams(ctypes.Structure):
+    """smre_admm_params of include/smre.h; defaults are App. B of the paper."""
+    _fields_ = [("sigma_psf", ctypes.c_float), ("rho1", ctypes.c_float), ("rho2", ctypes.c_float),
+                ("alpha1", ctypes.c_float), ("alpha2", ctypes.c_float), ("lam", ctypes.c_float),
+                ("gamma", ctypes.c_float), ("delta", ctypes.c_float), ("max_iter", ctypes.c_int),
+                ("n_sweeps", ctypes.c_int), ("check_every", ctypes.c_int)]
+
+
 exported_symbols = (
     "smre_create", "smre_project", "smre_project_host", "smre_destroy", "smre_set_schedule",
     "smre_info", "smre_family", "smre_export_increments", "smre_last_launch", "smre_last_error",
     "smre_plan_check", "smre_project_noalloc", "smre_project_tol", "smre_export_tile_cycles", "smre_calibrate", "smre_cumulant2",
+    "smre_shape", "smre_admm", "smre_psf_apply",
 )
 
 
@@ -66,6 +75,9 @@ def load_library(build_if_missing: bool = True):
                                    _vp, _vp, _vp, _vp]
     lib.smre_cumulant2.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]
     lib.smre_project_tol.argtypes = [_vp, _vp, _vp, ctypes.c_int, ctypes.c_float, _vp, _vp]
+    lib.smre_shape.argtypes = [_vp, _ip, _ip, _ip]
+    lib.smre_admm.argtypes = [_vp, ctypes.c_int, ctypes.c_int, _vp, ctypes.POINTER(AdmmParams), _vp, _vp, _ip, _vp, _vp]
+    lib.smre_psf_apply.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_float, _vp, _vp, _vp, _vp]
     lib.smre_export_tile_cycles.argtypes = [_vp, ctypes.c_int, _vp, _ip, _ip, _vp]
     for name in exported_symbols:
         getattr(lib, name).restype = ctypes.c_int
@@ -155,6 +167,47 @@ def calibrate(noise, sides, alpha):
 def smre_cumulant2(H, W, n_frames, stack_ptr, out_ptr, stream=0):
     """C_2 = <F^2> - <F>^2 per pixel over a stack (Eq. 19); device addresses."""
     _check(load_library().smre_cumulant2(int(H), int(W), int(n_frames), stack_ptr, out_ptr, stream))
+
+
+def smre_admm(handle, H, W, I_ptr, params, x_ptr, eps_ptr=None, hist_ptr=None, stream=0):
+    """The ADMM around the projection (include/smre.h); device addresses; returns the iterations done."""
+    it = ctypes.c_int(0)
+    _check(load_library().smre_admm(handle, int(H), int(W), I_ptr, ctypes.byref(params), x_ptr, eps_ptr,
+                                    ctypes.byref(it), hist_ptr, stream))
+    return it.value
+
+
+def smre_psf_apply(H, W, sigma, in_ptr, tmp_ptr, out_ptr, stream=0):
+    _check(load_library().smre_psf_apply(int(H), int(W), float(sigma), in_ptr, tmp_ptr, out_ptr, stream))
+
+
+def admm(solver, image, sigma_psf, gamma, delta=1e-3, max_iter=10000, n_sweeps=200, rho1=6.192, rho2=1.8, alpha1=1.2,
+         alpha2=0.12, lam=1.0, check_every=8, return_history=False):
+    """image: float32 CUDA tensor [H,W]; solver: a Solver with batch 1.  Returns (x, eps, iterations[, hist])."""
+    import torch
+    if not (image.is_cuda and image.dtype == torch.float32 and image.is_contiguous() and image.dim() == 2):
+        raise ValueError("image must be a contiguous float32 CUDA tensor [H,W]")
+    H, W = image.shape
+    p = AdmmParams(sigma_psf, rho1, rho2, alpha1, alpha2, lam, gamma, delta, int(max_iter), int(n_sweeps), int(check_every))
+    x = torch.empty_like(image)
+    eps = torch.empty_like(image)
+    hist = torch.zeros(2 * int(max_iter), device=image.device) if return_history else None
+    it = smre_admm(solver.handle, H, W, image.data_ptr(), p, x.data_ptr(), eps.data_ptr(),
+                   hist.data_ptr() if return_history else None, torch.cuda.current_stream(image.device).cuda_stream)
+    if return_history:
+        return x, eps, it, hist[:2 * it].reshape(it, 2)
+    return x, eps, it
+
+
+def psf_apply(image, sigma_psf):
+    import torch
+    if not (image.is_cuda and image.dtype == torch.float32 and image.is_contiguous() and image.dim() == 2):
+        raise ValueError("image must be a contiguous float32 CUDA tensor [H,W]")
+    tmp = torch.empty_like(image)
+    out = torch.empty_like(image)
+    smre_psf_apply(image.shape[0], image.shape[1], sigma_psf, image.data_ptr(), tmp.data_ptr(), out.data_ptr(),
+                   torch.cuda.current_stream(image.device).cuda_stream)
+    return out
 
 
 def cumulant2(stack):
