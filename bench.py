@@ -341,6 +341,73 @@ def run_gpu(args, w, rank, world):
         dist.destroy_process_group()
 
 
+def run_admm(args, w):
+    """--admm N: N iterations of the ADMM around the projection (smre_admm, NEXT-2) on the config's image (first frame
+    of a stack), App. B parameters, delta = 0 so that exactly N iterations run.  One GPU."""
+    import torch
+    import paper_1503_03492_b200 as smre
+    torch.cuda.set_device(0)
+    img = np.ascontiguousarray(w.y if w.y.ndim == 2 else w.y[0]).astype(np.float32)
+    n_sweeps = args.n_sweeps or 20
+    gamma = 8.0
+    sol = smre.Solver(w.H, w.W, w.sides, w.c, w.variant, 1)
+    I = torch.from_numpy(img).cuda()
+    for _ in range(max(1, args.warmup)):
+        smre.admm(sol, I, args.sigma, gamma=gamma, delta=0.0, max_iter=min(args.admm, 5), n_sweeps=n_sweeps)
+    sampler = ClockSampler(0)
+    sampler.start()
+    torch.cuda.synchronize()
+    evs = []
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        x, eps, it = smre.admm(sol, I, args.sigma, gamma=gamma, delta=0.0, max_iter=args.admm, n_sweeps=n_sweeps)
+        b.record()
+        evs.append((a, b))
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop()
+    dev = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+    iters = args.admm * args.steps
+    # the projection alone, same handle and sweep count
+    out = torch.empty_like(I)
+    sol.project(I, n_sweeps, out=out)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(20):
+        sol.project(I, n_sweeps, out=out)
+    b.record()
+    torch.cuda.synchronize()
+    proj_ms = a.elapsed_time(b) / 20
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import smre_oracle
+        t1 = time.perf_counter()
+        smre_oracle.admm(img, w.sides, w.c.astype(np.float64), 0 if w.variant == "standard" else 1, n_sweeps, args.sigma,
+                         6.192, 1.8, 1.2, 0.12, 1.0, gamma, 0.0, 2)
+        dt = time.perf_counter() - t1
+        cpu = {"value": 2 / dt, "unit": "iterations/s", "cores": 1, "kind": "oracle", "sample": "2 iterations of the same call",
+               "seconds": dt, **cpu_info()}
+    launches_per_iter = 6 + int(sol.last_launch[1])
+    print(json.dumps({
+        "metric": "admm_iterations_per_s", "value": iters / dev, "unit": "iterations/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dev / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name + "_admm", "variant": w.variant, "H": w.H, "W": w.W, "iterations_per_call": args.admm,
+                   "n_sweeps_per_projection": n_sweeps, "sigma_psf": args.sigma, "gamma": gamma,
+                   "parameters": "App. B: rho1 6.192, rho2 1.8, alpha1 1.2, alpha2 0.12, regularization 1",
+                   "note": "smre_admm (NEXT-2): host-synchronous call, delta = 0"},
+        "ms_per_iteration": dev / iters * 1e3, "projection_ms": proj_ms,
+        "projection_share": proj_ms / (dev / iters * 1e3),
+        "e2e": {"value": iters / wall, "unit": "iterations/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 8,
+                "note": "image resident; the call reads back the stop flag every 8 iterations"},
+        "gpu_launches": launches_per_iter * iters, "clocks": clocks, "roofline": None, "cpu_baseline": cpu,
+    }), flush=True)
+    sol.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -352,6 +419,8 @@ def main():
     ap.add_argument("--schedule", default="auto", choices=["auto", "graph", "persistent", "conveyor", "strips"])
     ap.add_argument("--ref-sweeps", type=int, default=200, help="oracle sample size in sweeps (~12 s on C1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--admm", type=int, default=None, help="time N iterations of smre_admm on the config's image instead")
+    ap.add_argument("--sigma", type=float, default=1.5, help="PSF standard deviation of --admm")
     ap.add_argument("--tol", type=float, default=None,
                     help="run smre_project_tol with this tolerance (n_sweeps = max) and report the iterations done")
     args = ap.parse_args()
@@ -360,6 +429,10 @@ def main():
     w = si.config(args.config, args.n_sweeps)
     if args.impl == "reference":
         run_reference(args, w, rank)
+        return
+    if args.admm is not None:
+        if rank == 0:
+            run_admm(args, w)
         return
     run_gpu(args, w, rank, world)
 
