@@ -292,6 +292,8 @@ struct ComputeState {
     float *tcol;                        // my column of the tile: tcol[t * pitch], t = tile row
     unsigned long long *box0;           // my column of slot 0 of my mailbox, addressed the same way
     long long slot_words, dest_step;    // next slot of my mailbox; same slot of the next strip's mailbox
+    unsigned long long *box_next;       // my column of the slot of the NEXT transition (built after the previous one)
+    bool mine;                          // my thread owns an image column
     unsigned *seen_sh;                  // shared memory [6]: cached progress words of strips j-3..j-1, j+1..j+3
                                         // (flow control of their mailbox rings)
 };
@@ -337,9 +339,9 @@ __device__ __forceinline__ void transition(const StripArgs &A, int pitch, int j,
     const long long c0 = clock64();
     cs.t_macro += c0 - cs.t_last;
 #endif
-    const bool mine = tid < A.W;
+    const bool mine = cs.mine;
     float *const trow = cs.tcol;                                // trow[t * pitch]: tile row t, my column
-    unsigned long long *const box = cs.box0 + (size_t)(mc & (ST_RING - 1)) * cs.slot_words;   // box[t * pitch]
+    unsigned long long *const box = cs.box_next;                // box[t * pitch]: slot mc % ST_RING of my mailbox
 
     // departures first: they are what the strips around are waiting for.  The plan is one 64-bit word, so the six
     // runs cost a few ALU instructions each and no dependent shared-memory loads.
@@ -404,6 +406,10 @@ __device__ __forceinline__ void transition(const StripArgs &A, int pitch, int j,
 #endif
     bar_sync(2, NT);
     if (tid == 0) st_relaxed_gpu32(A.done + (size_t)cta * 32, tag);   // my mailbox slot of this transition is free again
+    // the next transition's slot, built now and kept (it was rebuilt from the kernel parameters and %ctaid in front
+    // of the sends, on the critical path of the strips around)
+    cs.box_next = cs.box0 + (size_t)((mc + 1) & (ST_RING - 1)) * cs.slot_words;
+    asm volatile("" : "+l"(cs.box_next));
 #ifdef SMRE_ST_KO
     const long long c3 = clock64();
     cs.t_send += c1 - c0; cs.t_recv += c2 - c1; cs.t_bar += c3 - c2; cs.t_last = c3;
@@ -782,6 +788,8 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
         cs.slot_words = (long long)st_tile_rows(T) * pitch;
         cs.box0 = A.mail + (long long)cta * ST_RING * cs.slot_words + tid;
         cs.dest_step = st_dest_step(A);
+        cs.box_next = cs.box0 + cs.slot_words;                   // transition 1 uses slot 1
+        cs.mine = tid < W;
         Waiter wt(A, abort_flag);
         bool stopped_early = false;
         const int h_lo = tab[0].hold_lo, h_hi = tab[0].hold_hi;      // rows held at the top of EVERY sweep
