@@ -182,6 +182,18 @@ struct __align__(16) MacroEntry {
     // first row in bits 0-3, number of rows in bits 4-9; splan: the six send runs (k = 0..5), rplan: the two arrival runs
     unsigned long long splan, rplan;
 };
+// The hand-off behind a macro step as a ready-made program (built once at kernel start): with every compute warp in
+// the hand-off, the time it takes is set by the instructions the warps issue in front of and behind the one L2
+// round trip, so nothing is decoded or multiplied there any more.
+struct __align__(16) HandProg {
+    int send_doff[3];           // run i: mailbox word offset of its first word from (slot, tile row 0, my column) of MY
+                                // mailbox: d * dest_step + row * pitch
+    unsigned send_meta[3];      // run i: tile row | rows << 8 | direction index k << 16
+    unsigned counts;            // send runs | arriving rows << 8 | (more than 3 send runs: take the plan words) << 16
+    unsigned recv_rows[4];      // the arriving tile rows, one byte each
+    unsigned pad;
+};
+static_assert(sizeof(HandProg) == 48, "HandProg");
 static_assert(sizeof(MacroEntry) == 96 && offsetof(MacroEntry, splan) % 16 == 0, "MacroEntry");
 
 // ------------------------------------------------------------------------------------------------ window sums
@@ -327,7 +339,7 @@ __device__ __forceinline__ void st_ring_space(const StripArgs &A, int cta, int d
 // the hand-offs of one transition cannot form a cycle.  A thread owns column tid (W <= compute threads).
 // A row travels to slot (receiver's tile row) of the receiver's mailbox, whoever sends it.
 __device__ __forceinline__ void transition(const StripArgs &A, int pitch, int j, int cta, unsigned long long splan,
-                                           unsigned long long rplan, ComputeState &cs, int tid, int NT, Waiter &w)
+                                           const HandProg *prog, ComputeState &cs, int tid, int NT, Waiter &w)
 {
     constexpr int MAXR = 8;                                    // rows requested at once
     static_assert(ST_HOPS == 3, "the sends below are written out for three hops");
@@ -342,23 +354,33 @@ __device__ __forceinline__ void transition(const StripArgs &A, int pitch, int j,
     const bool mine = cs.mine;
     float *const trow = cs.tcol;                                // trow[t * pitch]: tile row t, my column
     unsigned long long *const box = cs.box_next;                // box[t * pitch]: slot mc % ST_RING of my mailbox
+    const uint4 p0 = reinterpret_cast<const uint4 *>(prog)[0];   // send_doff[0..2], send_meta[0]
+    const uint4 p1 = reinterpret_cast<const uint4 *>(prog)[1];   // send_meta[1..2], counts, recv_rows[0]
+    const unsigned counts = p1.z;
 
-    // departures first: they are what the strips around are waiting for.  The plan is one 64-bit word, so the six
-    // runs cost a few ALU instructions each and no dependent shared-memory loads.
-    if (splan != 0ull) {
-#pragma unroll
+    // departures first: they are what the strips around are waiting for
+    auto send_run = [&](int k, int row, int n, unsigned long long *dst) {
+        const int d = k < ST_HOPS ? k - ST_HOPS : k - ST_HOPS + 1;
+        unsigned seen = *(volatile unsigned *)(cs.seen_sh + k);
+        st_ring_space(A, cta, d, tag, mc, seen, w);
+        if (!mine) return;
+        const float *src = trow + row * pitch;
+#pragma unroll 1
+        for (int r = 0; r < n; ++r) st_relaxed_gpu64(dst + r * pitch, pack_word(tag, src[r * pitch]));
+    };
+    if (counts & 0xff0000u) {                                   // more than three runs (does not happen at T = 4, 8)
+#pragma unroll 1
         for (int k = 0; k < 2 * ST_HOPS; ++k) {
             const unsigned f = (unsigned)(splan >> (10 * k)) & 1023u;
             if (f == 0u) continue;
             const int d = k < ST_HOPS ? k - ST_HOPS : k - ST_HOPS + 1;
-            unsigned seen = *(volatile unsigned *)(cs.seen_sh + k);
-            st_ring_space(A, cta, d, tag, mc, seen, w);
-            if (!mine) continue;
-            const int lo = (int)(f & 15u), n = (int)(f >> 4);
-            unsigned long long *dst = box + d * cs.dest_step + lo * pitch;
-            const float *src = trow + lo * pitch;
-            for (int r = 0; r < n; ++r) st_relaxed_gpu64(dst + r * pitch, pack_word(tag, src[r * pitch]));
+            send_run(k, (int)(f & 15u), (int)(f >> 4), box + d * cs.dest_step + (int)(f & 15u) * pitch);
         }
+    } else {
+        const int nsend = (int)(counts & 255u);
+        if (nsend > 0) send_run((int)(p0.w >> 16), (int)(p0.w & 255u), (int)(p0.w >> 8) & 255, box + (int)p0.x);
+        if (nsend > 1) send_run((int)(p1.x >> 16), (int)(p1.x & 255u), (int)(p1.x >> 8) & 255, box + (int)p0.y);
+        if (nsend > 2) send_run((int)(p1.y >> 16), (int)(p1.y & 255u), (int)(p1.y >> 8) & 255, box + (int)p0.z);
     }
 #ifdef SMRE_ST_KO
     const long long c1 = clock64();
@@ -370,20 +392,21 @@ __device__ __forceinline__ void transition(const StripArgs &A, int pitch, int j,
     const bool asks = tid < 2 * ST_HOPS && j + nd >= 0 && j + nd < A.NS;
     if (asks) s_new = ld_relaxed_gpu32(A.done + (size_t)(cta + nd) * 32);
 
-    // arrivals: up to two runs of consecutive tile rows.  All words of a batch are requested at once; a word whose
-    // tag is right goes to the tile, the others are requested again.
-    if (mine && rplan != 0ull) {
-        const int lo0 = (int)(rplan & 15u), n0 = (int)(rplan >> 4) & 63, lo1 = (int)(rplan >> 10) & 15, n = n0 + ((int)(rplan >> 14) & 63);
+    // arrivals: all words of a batch are requested at once; a word whose tag is right goes to the tile, the others
+    // are requested again
+    const int nrecv = (int)(counts >> 8) & 255;
+    if (mine && nrecv > 0) {
         w.begin();
-        for (int r0 = 0; r0 < n; r0 += MAXR) {
+#pragma unroll 1
+        for (int r0 = 0; r0 < nrecv; r0 += MAXR) {
+            unsigned lo4 = p1.w, hi4;                            // rows r0 .. r0 + 3, r0 + 4 .. r0 + 7
+            if (r0 == 0) hi4 = prog->recv_rows[1];
+            else { lo4 = prog->recv_rows[2]; hi4 = prog->recv_rows[3]; }
             int off[MAXR];
-            unsigned missing = 0;
 #pragma unroll
-            for (int r = 0; r < MAXR; ++r) {
-                const int i = r0 + r;
-                off[r] = (i < n0 ? lo0 + i : lo1 + (i - n0)) * pitch;
-                if (i < n) missing |= 1u << r;
-            }
+            for (int r = 0; r < MAXR; ++r) off[r] = (int)(((r < 4 ? lo4 : hi4) >> (8 * (r & 3))) & 255u) * pitch;
+            const int cnt = nrecv - r0;
+            unsigned missing = cnt >= MAXR ? (1u << MAXR) - 1u : (1u << cnt) - 1u;
             for (;;) {
                 unsigned long long wd[MAXR];
 #pragma unroll
@@ -706,6 +729,7 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
     unsigned *stopped = abort_flag + 3;                         // tol mode: the stop rule has fired
     double *wsum = reinterpret_cast<double *>(abort_flag + 4);  // [ST_MAX_WARPS + 1] per-warp parts of ||x_r - x_{r-1}||^2
     unsigned *seen_sh = reinterpret_cast<unsigned *>(wsum + ST_MAX_WARPS + 2);   // [2 * ST_HOPS], see transition()
+    HandProg *prog = reinterpret_cast<HandProg *>(seen_sh + 8);  // [macro steps]: the hand-off behind each of them
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int NWC = A.NWC, NT = NWC * 32, NTL = NT + (ST_KO(A, 32) ? 0 : 32);
@@ -754,6 +778,27 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
             if (e.recv_hi[i] > e.recv_lo[i])
                 e.rplan |= (unsigned long long)((e.recv_lo[i] + tb) | ((e.recv_hi[i] - e.recv_lo[i]) << 4)) << (10 * i);
         tab[threadIdx.x] = e;
+        HandProg hp;
+        const int dest_step = (int)st_dest_step(A);
+        int ns = 0, nr = 0;
+        unsigned general = 0;
+        for (int i = 0; i < 3; ++i) { hp.send_doff[i] = 0; hp.send_meta[i] = 0; }
+        for (int i = 0; i < 4; ++i) hp.recv_rows[i] = 0;
+        for (int k = 0; k < 2 * ST_HOPS; ++k) {
+            const int n = e.send_hi[k] - e.send_lo[k];
+            if (n <= 0) continue;
+            if (ns == 3) { general = 1; continue; }
+            const int d = k < ST_HOPS ? k - ST_HOPS : k - ST_HOPS + 1, row = e.send_lo[k] + tb;
+            hp.send_doff[ns] = d * dest_step + row * pitch;
+            hp.send_meta[ns] = (unsigned)row | (unsigned)n << 8 | (unsigned)k << 16;
+            ++ns;
+        }
+        for (int i = 0; i < 2; ++i)
+            for (int y = e.recv_lo[i]; y < e.recv_hi[i]; ++y, ++nr)
+                if (nr < 16) hp.recv_rows[nr >> 2] |= (unsigned)(y + tb) << (8 * (nr & 3));
+        hp.counts = (unsigned)ns | (unsigned)nr << 8 | general << 16;
+        hp.pad = 0;
+        prog[threadIdx.x] = hp;
     }
     if (threadIdx.x == 0) {
         for (int i = 0; i < ST_NSTG; ++i) mbar_init(&full[i], 1);
@@ -842,7 +887,7 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
             }
             for (int m = 0; m < M; ++m) {
                 const MacroEntry e = tab[m];
-                const unsigned long long splan = e.splan, rplan = e.rplan;
+                const unsigned long long splan = e.splan;
                 const bool staged = sweep > 0 && !ST_KO(A, 2);
                 const bool handoff = !(m + 1 == M && sweep + 1 == A.n_sweeps);   // none after the very last one
 #define SMRE_RUN(S_)                                                                                                   \
@@ -852,7 +897,7 @@ __global__ void __launch_bounds__(MAXT, 1) strips_kernel(const __grid_constant__
                 }
 #undef SMRE_RUN
                 if (!handoff) break;
-                transition(A, pitch, j, cta, splan, rplan, cs, tid, NT, wt);
+                transition(A, pitch, j, cta, splan, prog + m, cs, tid, NT, wt);
             }
         }
         if (A.tol_mode && !stopped_early && j == 0 && tid == 0 && A.sweeps_done) A.sweeps_done[frame] = A.n_sweeps;
@@ -909,7 +954,7 @@ static void set_why(char *why, size_t n, const char *fmt, ...)
     va_end(ap);
 }
 
-static size_t strips_fixed_smem() { return ST_NSTG * 8 + ST_MAX_SIDES * ST_MAX_SIDE * sizeof(MacroEntry) + 16 + (ST_MAX_WARPS + 2) * 8 + 32; }
+static size_t strips_fixed_smem() { return ST_NSTG * 8 + ST_MAX_SIDES * ST_MAX_SIDE * sizeof(MacroEntry) + 16 + (ST_MAX_WARPS + 2) * 8 + 32 + ST_MAX_SIDES * ST_MAX_SIDE * sizeof(HandProg); }
 
 // Brute-force check of one strip height against every geometry of a sweep (host only, closed forms).
 static bool strips_check_T(int H, int NS, int T, const int *sides, int n_sides, int *max_rows, int *max_hop,
