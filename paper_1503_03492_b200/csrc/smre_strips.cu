@@ -395,31 +395,38 @@ __device__ __forceinline__ void transition(const StripArgs &A, int pitch, int j,
     // arrivals: all words of a batch are requested at once; a word whose tag is right goes to the tile, the others
     // are requested again
     const int nrecv = (int)(counts >> 8) & 255;
+    auto recv_batch = [&](auto rtag, unsigned lo4, unsigned hi4, int cnt) {
+        constexpr int R = decltype(rtag)::value;                // rows requested at once
+        int off[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) off[r] = (int)(((r < 4 ? lo4 : hi4) >> (8 * (r & 3))) & 255u) * pitch;
+        unsigned missing = cnt >= R ? (1u << R) - 1u : (1u << cnt) - 1u;
+        for (;;) {
+            unsigned long long wd[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if (missing >> r & 1u) wd[r] = ld_relaxed_gpu64(box + off[r]);
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if ((missing >> r & 1u) && (unsigned)(wd[r] >> 32) == tag) {
+                    trow[off[r]] = __uint_as_float((unsigned)wd[r]);
+                    missing &= ~(1u << r);
+                }
+            if (ST_KO(A, 64)) missing = 0;
+            if (!missing || w.slow(ST_W_MAIL)) break;
+        }
+    };
     if (mine && nrecv > 0) {
         w.begin();
+        if (nrecv <= 2) {                                       // the usual case: one row per moving boundary
+            recv_batch(std::integral_constant<int, 2>{}, p1.w, 0u, nrecv);
+        } else {
 #pragma unroll 1
-        for (int r0 = 0; r0 < nrecv; r0 += MAXR) {
-            unsigned lo4 = p1.w, hi4;                            // rows r0 .. r0 + 3, r0 + 4 .. r0 + 7
-            if (r0 == 0) hi4 = prog->recv_rows[1];
-            else { lo4 = prog->recv_rows[2]; hi4 = prog->recv_rows[3]; }
-            int off[MAXR];
-#pragma unroll
-            for (int r = 0; r < MAXR; ++r) off[r] = (int)(((r < 4 ? lo4 : hi4) >> (8 * (r & 3))) & 255u) * pitch;
-            const int cnt = nrecv - r0;
-            unsigned missing = cnt >= MAXR ? (1u << MAXR) - 1u : (1u << cnt) - 1u;
-            for (;;) {
-                unsigned long long wd[MAXR];
-#pragma unroll
-                for (int r = 0; r < MAXR; ++r)
-                    if (missing >> r & 1u) wd[r] = ld_relaxed_gpu64(box + off[r]);
-#pragma unroll
-                for (int r = 0; r < MAXR; ++r)
-                    if ((missing >> r & 1u) && (unsigned)(wd[r] >> 32) == tag) {
-                        trow[off[r]] = __uint_as_float((unsigned)wd[r]);
-                        missing &= ~(1u << r);
-                    }
-                if (ST_KO(A, 64)) missing = 0;
-                if (!missing || w.slow(ST_W_MAIL)) break;
+            for (int r0 = 0; r0 < nrecv; r0 += MAXR) {
+                unsigned lo4 = p1.w, hi4;                        // rows r0 .. r0 + 3, r0 + 4 .. r0 + 7
+                if (r0 == 0) hi4 = prog->recv_rows[1];
+                else { lo4 = prog->recv_rows[2]; hi4 = prog->recv_rows[3]; }
+                recv_batch(std::integral_constant<int, MAXR>{}, lo4, hi4, nrecv - r0);
             }
         }
     }
