@@ -414,6 +414,7 @@ __device__ __forceinline__ void transition(const StripArgs &A, int pitch, int j,
                 }
             if (ST_KO(A, 64)) missing = 0;
             if (!missing || w.slow(ST_W_MAIL)) break;
+            if (w.spins > 2u) __nanosleep(256);                 // a long wait (an idle strip): stop hammering L2
         }
     };
     if (mine && nrecv > 0) {
