@@ -266,12 +266,21 @@ __device__ __forceinline__ void band_group(float *xt, const float *qs, float *qg
             n2[i] = fmaf(v[i][r], v[i][r], n2[i]);
         }
     }
-#pragma unroll
-    for (int i = 0; i < G; ++i) al[i] = ball_scale(window_total<S>(n2[i], src), cth, sq);
+    // The decision "does this column change memory" does not wait for the scale factor: the window is scaled iff its
+    // sum exceeds the threshold (the compare of ball_scale), which is known as soon as the shuffle tree is through;
+    // the reciprocal square root and the products are only formed for the columns that go on.  (A window that is
+    // scaled by a factor that rounds to exactly 1 is updated too: x' = v, q' = 0, what memory holds if q was 0.)
+    bool go[G];
 #pragma unroll
     for (int i = 0; i < G; ++i) {
-        const bool live = !elim || !HAS_Q || al[i] != 1.0f || (qbits[i] << 1) != 0u;
-        if (on && (i == 0 || i < nvalid) && live) {
+        al[i] = window_total<S>(n2[i], src);                    // the sum for now
+        const bool carried = !elim || !HAS_Q || (qbits[i] << 1) != 0u;
+        go[i] = on && (i == 0 || i < nvalid) && (carried || al[i] > cth);
+    }
+#pragma unroll
+    for (int i = 0; i < G; ++i) {
+        if (go[i]) {
+            al[i] = ball_scale(al[i], cth, sq);
 #pragma unroll
             for (int r = 0; r < S; ++r) {
                 float xn, qn;
