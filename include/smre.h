@@ -213,8 +213,8 @@ smre_status smre_calibrate(int H, int W, int n_frames, const int *sides, int n_s
  */
 smre_status smre_cumulant2(int H, int W, int n_frames, const float *stack_dev, float *c2_out_dev, void *cuda_stream);
 
-/* Shape the handle was created for (any pointer may be NULL). */
-smre_status smre_shape(smre_handle h, int *H, int *W, int *batch);
+/* Shape and variant the handle was created for (any pointer may be NULL). */
+smre_status smre_shape(smre_handle h, int *H, int *W, int *batch, int *variant);
 
 /* ---- The ADMM around the projection (Alg. 1, Eq. 9-13) -----------------
  * Solves Eq. 10,  min G(eps) + (lambda/2) ||z||^2  s.t.  I = A * x + eps,  z = x,  with G the multi-resolution
@@ -235,7 +235,9 @@ smre_status smre_shape(smre_handle h, int *H, int *W, int *batch);
  *   I_dev         [H][W] device, read only;  x_out_dev [H][W] device: the estimate x;  eps_out_dev: the residual, or NULL
  *   iters_out     HOST int, or NULL: iterations done
  *   hist_out_dev  device [2 * max_iter] or NULL: the two norms after every iteration
- * Synchronous (returns after the stream has drained).  Allocates and frees its workspace (10 images) per call.
+ * Synchronous: it runs behind the work already queued on cuda_stream, on a stream of its own, and returns when it
+ * has finished (with the incomplete variant one iteration is replayed as a CUDA graph).  Allocates and frees its
+ * workspace (10 images) per call.
  * Errors: SMRE_EINVAL (pointers, shape mismatch, batch != 1, parameters out of range), SMRE_EUNSUPPORTED
  * (sigma_psf > 10.6), SMRE_ENOMEM, SMRE_ECUDA, and whatever smre_project returns. */
 typedef struct {

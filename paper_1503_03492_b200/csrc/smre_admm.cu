@@ -196,12 +196,23 @@ extern "C" smre_status smre_admm(smre_handle h, int H, int W, const float *I_dev
     if (!(p->rho1 > 0.0f) || !(p->rho2 > 0.0f) || !(p->gamma > 0.0f) || p->lambda < 0.0f || p->sigma_psf < 0.0f ||
         p->max_iter <= 0 || p->n_sweeps <= 0 || !(p->delta >= 0.0f))
         return fail(SMRE_EINVAL, "smre_admm: rho1, rho2, gamma > 0, lambda, sigma_psf, delta >= 0, max_iter, n_sweeps >= 1");
-    int hH = 0, hW = 0, hB = 0;
-    if (smre_shape(h, &hH, &hW, &hB) != SMRE_OK) return SMRE_EINVAL;
+    int hH = 0, hW = 0, hB = 0, hvariant = 0;
+    if (smre_shape(h, &hH, &hW, &hB, &hvariant) != SMRE_OK) return SMRE_EINVAL;
     if (hH != H || hW != W || hB != 1) return fail(SMRE_EINVAL, "smre_admm: H, W must be the handle's and its batch must be 1");
     Taps t;
     if (!make_taps(p->sigma_psf, t)) return fail(SMRE_EUNSUPPORTED, "smre_admm: sigma_psf beyond the compiled limit (radius 32)");
-    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // The call is synchronous, so it runs on a stream of its own behind the work already queued on the caller's
+    // stream: that stream can be captured (the caller's may be the legacy default stream, which cannot), and with the
+    // incomplete variant one iteration is eleven small launches whose launch cost exceeds their run time.
+    cudaStream_t user_st = (cudaStream_t)cuda_stream, st = nullptr;
+    cudaEvent_t ev = nullptr;
+    if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventRecord(ev, user_st) != cudaSuccess || cudaStreamWaitEvent(st, ev, 0) != cudaSuccess) {
+        if (ev) cudaEventDestroy(ev);
+        if (st) cudaStreamDestroy(st);
+        return fail(SMRE_ECUDA, "smre_admm: could not create its stream");
+    }
     const size_t N = (size_t)H * W;
     const dim3 block(128), grid((W + 127) / 128, H);
     const int blocks = (int)(grid.x * grid.y);
@@ -229,17 +240,33 @@ extern "C" smre_status smre_admm(smre_handle h, int H, int W, const float *I_dev
         S.inv2gamma = 1.0f / (2.0f * p->gamma); S.delta = p->delta;
         e = cudaMemsetAsync(flags, 0, 2 * sizeof(int), st);
         if (e == cudaSuccess) { admm_init_kernel<<<grid, block, 0, st>>>(S); e = cudaGetLastError(); }
+        auto iteration = [&]() -> smre_status {
+            admm_rows_kernel<<<grid, block, 0, st>>>(S.w, S.tmp, H, W, t, S.stopped);
+            admm_x_update_kernel<<<grid, block, 0, st>>>(S, t);
+            admm_rows_kernel<<<grid, block, 0, st>>>(S.x, S.tmp, H, W, t, S.stopped);
+            admm_residual_kernel<<<grid, block, 0, st>>>(S, t);
+            const smre_status r = smre_project(h, S.X, S.eps_next, p->n_sweeps, (void *)st);
+            admm_dual_kernel<<<grid, block, 0, st>>>(S);
+            admm_decide_kernel<<<1, 256, 0, st>>>(S);
+            return r;
+        };
+        // incomplete variant: one iteration as a CUDA graph (plain launches only; the standard variant's projection is
+        // one cooperative launch that dwarfs the rest, it stays as it is)
+        cudaGraphExec_t exec = nullptr;
+        if (e == cudaSuccess && hvariant == (int)SMRE_INCOMPLETE && cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            const smre_status r = iteration();
+            cudaGraph_t g = nullptr;
+            const cudaError_t ce = cudaStreamEndCapture(st, &g);
+            if (r != SMRE_OK || ce != cudaSuccess || !g || cudaGraphInstantiate(&exec, g, 0) != cudaSuccess) exec = nullptr;
+            if (g) cudaGraphDestroy(g);
+            cudaGetLastError();
+        }
         int done = 0;
         while (e == cudaSuccess && rc == SMRE_OK && done < p->max_iter) {
             const int n = p->max_iter - done < check_every ? p->max_iter - done : check_every;
             for (int k = 0; k < n && rc == SMRE_OK; ++k) {
-                admm_rows_kernel<<<grid, block, 0, st>>>(S.w, S.tmp, H, W, t, S.stopped);
-                admm_x_update_kernel<<<grid, block, 0, st>>>(S, t);
-                admm_rows_kernel<<<grid, block, 0, st>>>(S.x, S.tmp, H, W, t, S.stopped);
-                admm_residual_kernel<<<grid, block, 0, st>>>(S, t);
-                rc = smre_project(h, S.X, S.eps_next, p->n_sweeps, cuda_stream);
-                admm_dual_kernel<<<grid, block, 0, st>>>(S);
-                admm_decide_kernel<<<1, 256, 0, st>>>(S);
+                if (exec) { if (cudaGraphLaunch(exec, st) != cudaSuccess) rc = fail(SMRE_ECUDA, "smre_admm: graph launch failed"); }
+                else rc = iteration();
             }
             done += n;
             if (rc != SMRE_OK) break;
@@ -256,11 +283,15 @@ extern "C" smre_status smre_admm(smre_handle h, int H, int W, const float *I_dev
             if (e == cudaSuccess && iters_out) *iters_out = flags_host[0];
         }
         if (e != cudaSuccess && rc == SMRE_OK) rc = fail(SMRE_ECUDA, cudaGetErrorString(e));
+        if (exec) cudaGraphExecDestroy(exec);
     }
+    cudaStreamSynchronize(st);
     if (ws) cudaFree(ws);
     if (parts) cudaFree(parts);
     if (flags) cudaFree(flags);
     if (flags_host) cudaFreeHost(flags_host);
+    cudaEventDestroy(ev);
+    cudaStreamDestroy(st);
     return rc;
 }
 

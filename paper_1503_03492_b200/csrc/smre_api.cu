@@ -365,12 +365,13 @@ extern "C" smre_status smre_project_host(smre_handle h, const float *y_host, flo
     return SMRE_OK;
 }
 
-extern "C" smre_status smre_shape(smre_handle h, int *H, int *W, int *batch)
+extern "C" smre_status smre_shape(smre_handle h, int *H, int *W, int *batch, int *variant)
 {
     if (!h) { set_last_error("smre_shape: null handle"); return SMRE_EINVAL; }
     if (H) *H = h->H;
     if (W) *W = h->W;
     if (batch) *batch = h->B;
+    if (variant) *variant = (int)h->variant;
     return SMRE_OK;
 }
 

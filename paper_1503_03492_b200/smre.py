@@ -75,7 +75,7 @@ def load_library(build_if_missing: bool = True):
                                    _vp, _vp, _vp, _vp]
     lib.smre_cumulant2.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]
     lib.smre_project_tol.argtypes = [_vp, _vp, _vp, ctypes.c_int, ctypes.c_float, _vp, _vp]
-    lib.smre_shape.argtypes = [_vp, _ip, _ip, _ip]
+    lib.smre_shape.argtypes = [_vp, _ip, _ip, _ip, _ip]
     lib.smre_admm.argtypes = [_vp, ctypes.c_int, ctypes.c_int, _vp, ctypes.POINTER(AdmmParams), _vp, _vp, _ip, _vp, _vp]
     lib.smre_psf_apply.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_float, _vp, _vp, _vp, _vp]
     lib.smre_export_tile_cycles.argtypes = [_vp, ctypes.c_int, _vp, _ip, _ip, _vp]
